@@ -1,0 +1,160 @@
+/*
+ * hermes.h -- C ABI of the B200-native HERMES per-chunk hierarchical KV-cache update
+ *             (arXiv 2601.14724; citations are PAPER.md:<line> + equation).
+ *
+ * One call of hermes_append_chunk() is one chunk arrival (Fig. 3 at :61):
+ *   a0 append the chunk's K/V after the cached tokens of every layer;
+ *   a1 attention importance W of every cached video token w.r.t. the guidance-prompt
+ *      pseudo-query (Eq. 2), middle + deep layers only;
+ *   a2 normalise, recency (Eq. 1) and layer weighting (Eq. 3-4);
+ *   a3 cross-layer memory smoothing (Eq. 5; lambda of Eq. 7);
+ *   a4 per-layer Top-K under the budget |M| (Eq. 6);
+ *   a5 gather-compaction K_l[I_l], V_l[I_l] (Eq. 6);
+ *   a6 eager position re-indexing (Eq. 8; M-RoPE Eq. 11);
+ *   a7 delta rotary correction of the kept keys (Eq. 9-10; Eq. 12-13, :629-634).
+ * Every step runs in sm_100a CUDA kernels; there is no CPU fallback.
+ *
+ * Conventions
+ *   - All functions return HERMES_OK (0) or a negative hermes_status; they never throw, abort or print.
+ *   - "device pointer" = memory of the CUDA device in hermes_config.device; "host pointer" = CPU memory.
+ *   - Tensors are dense, row-major, element type hermes_config.dtype (fp32 or bf16).
+ *   - Calls are stream-ordered and asynchronous: they enqueue work on `cuda_stream` (a cudaStream_t;
+ *     NULL = the legacy default stream) and return; no host synchronisation on the success path.
+ *     Caller buffers must stay valid and unmodified until the stream has passed the call.
+ *   - The library allocates no device memory: the caller provides one workspace of
+ *     hermes_workspace_bytes() bytes (256-byte aligned), which the handle owns until hermes_destroy().
+ *   - Query head h uses KV head h / (n_q_heads / n_kv_heads) (grouped-query attention).
+ *   - A handle is not thread-safe; use one per host thread or serialise calls.
+ */
+#ifndef HERMES_H_
+#define HERMES_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  HERMES_OK = 0,
+  HERMES_EINVAL = -1,     /* bad argument / unsupported geometry; state unchanged            */
+  HERMES_ECAPACITY = -2,  /* len + n_new exceeds max_tokens (or workspace too small)          */
+  HERMES_ESTATE = -3,     /* call not valid in the handle's current state                     */
+  HERMES_ECUDA = -4,      /* a CUDA runtime / driver call failed (no device, launch error...) */
+  HERMES_ENOMEM = -5      /* host allocation failed                                           */
+} hermes_status;
+
+enum { HERMES_F32 = 0, HERMES_BF16 = 1 };
+enum { HERMES_ROPE_1D = 0, HERMES_ROPE_M3D = 1 };   /* App. E.1 / App. E.2                    */
+enum { HERMES_NORM_MAX = 0, HERMES_NORM_SUM = 1 };  /* alpha of Eq. 1/2 (DESIGN c2)           */
+enum { HERMES_SCORE_AUTO = 0, HERMES_SCORE_SIMT = 1, HERMES_SCORE_TCGEN05 = 2 };
+
+typedef struct hermes hermes_t;  /* opaque; owns n_streams x n_layers double-buffered caches   */
+
+typedef struct {
+  int32_t n_layers, n_q_heads, n_kv_heads;
+  int32_t head_dim;             /* 32, 64 or 128                                              */
+  int32_t dtype;                /* HERMES_F32 | HERMES_BF16: K, V and Q_probe element type     */
+  int32_t n_streams;            /* B independent streams advanced by every call                */
+  int32_t tokens_per_frame;     /* N_f; informational                                          */
+  int32_t budget;               /* |M| tokens kept per layer                    */
+  int32_t max_chunk_tokens;     /* largest n_new                                               */
+  int32_t max_tokens;           /* slots per layer; 0 -> budget + max_chunk_tokens             */
+  int32_t max_probe_tokens;     /* largest n_probe                                             */
+  int32_t n_shallow, n_deep;    /* -1 -> max(1, round(0.1 L)), max(1, round(0.3 L)) */
+  int32_t l_short, l_long;      /* -1 -> first / last middle layer (Eq. 3)                     */
+  float omega0, gamma;          /* Eq. 3: 0.75, 0.6                              */
+  float forget_rate;            /* k > 0 of Eq. 1, per token of temporal distance              */
+  int32_t norm_mode;            /* HERMES_NORM_*                                               */
+  float lambda_shallow, lambda_middle, lambda_deep; /* Eq. 7: 0.1, 0.3, 0.4                    */
+  float softmax_scale;          /* 0 -> 1/sqrt(head_dim)                                       */
+  int32_t rope_mode;            /* HERMES_ROPE_*                                               */
+  float rope_theta;             /* RoPE base; theta_j = base^(-2j/head_dim)                    */
+  int32_t mrope_section[3];     /* rotary pairs owned by (t, h, w); sum = head_dim/2           */
+  int32_t mrope_compact_axes;   /* bit0 t, bit1 h, bit2 w: axes re-indexed by Eq. 11           */
+  int32_t mrope_grid_h, mrope_grid_w; /* merged patch grid; tokens per temporal step = h*w     */
+  int32_t pos_offset;           /* length of the fixed system prefix            */
+  int32_t score_path;           /* HERMES_SCORE_*: AUTO picks tcgen05 when the contraction is dense */
+  int32_t device;               /* CUDA device ordinal                                         */
+} hermes_config;
+
+/* Borrowed DEVICE pointers into the workspace for one (stream, layer); valid until the next
+ * hermes_append_chunk*() or hermes_destroy() on the handle.  Contents are defined once the stream of the
+ * last append has been synchronised.                                                                  */
+typedef struct {
+  const void *k, *v;            /* [len, n_kv_heads, head_dim], token-major                    */
+  const int32_t *pos;           /* [n_axes][pos_stride]; first `len` entries of each axis valid */
+  int32_t n_axes;               /* 1 (1D RoPE) or 3 (M-RoPE: t, h, w)                          */
+  int32_t pos_stride;
+  int32_t len;                  /* host-tracked: min(tokens appended, budget) after an eviction */
+  const float *last_scores;     /* [last_T] smoothed scores S~ of the last eviction, else NULL  */
+  const int32_t *last_kept;     /* [budget] ascending indices I_l into the last candidate list  */
+  int32_t last_T;               /* candidates of the last eviction (0 if none yet)              */
+} hermes_cache_view;
+
+/* Defaults of the paper for everything but geometry; geometry fields are 0. */
+void hermes_default_config(hermes_config *cfg);
+
+/* Bytes of device workspace a handle with this config needs; 0 if the config is invalid.              */
+size_t hermes_workspace_bytes(const hermes_config *cfg);
+
+/* Validates cfg (HERMES_EINVAL: H_q % H_kv != 0, head_dim not in {32,64,128}, sum(mrope_section) !=
+ * head_dim/2, budget <= 0, forget_rate <= 0, n_shallow + n_deep > L, ...), binds `workspace`
+ * (device pointer, `bytes` >= hermes_workspace_bytes, else HERMES_ECAPACITY), builds the rotary table
+ * on `cfg->device`.  HERMES_ECUDA if no usable sm_100 device.  *out is NULL on failure.
+ * This call synchronises the device once.                                                            */
+int hermes_create(const hermes_config *cfg, void *workspace, size_t bytes, hermes_t **out);
+
+/* One chunk arrival for all B streams.
+ *   K_new, V_new : device, [B, L, n_new, H_kv, d]; K is post-RoPE at the arrival positions.
+ *   Q_probe      : device, [B, L, H_q, n_probe, d] post-RoPE guidance-prompt query states, or NULL.
+ *                  Slices of shallow layers are never read.
+ *   pos_start    : 1D: position of the chunk's token 0 (token j sits at pos_start + j); M-RoPE: temporal
+ *                  index of the chunk's first step.  -1 -> default: 1D pos_offset + len; M-RoPE
+ *                  pos_offset + min(temporal steps seen, budget).  Must exceed every cached position.
+ * With T = len + n_new: if Q_probe == NULL or T <= budget the chunk is only appended;
+ * otherwise steps a1-a7 run and len becomes budget.  T > max_tokens -> HERMES_ECAPACITY, state unchanged. */
+int hermes_append_chunk(hermes_t *h, const void *K_new, const void *V_new, const void *Q_probe,
+                        int32_t n_new, int32_t n_probe, int32_t pos_start, void *cuda_stream);
+
+/* Same update with HOST buffers (pinned memory recommended): stages K_new/V_new/Q_probe to the device
+ * with cudaMemcpyAsync on `cuda_stream`, runs the update, and, if kept_out != NULL, copies the kept
+ * index lists I_l [B, L, budget] int32 back to the host (only meaningful when an eviction ran).        */
+int hermes_append_chunk_host(hermes_t *h, const void *K_new_host, const void *V_new_host,
+                             const void *Q_probe_host, int32_t n_new, int32_t n_probe,
+                             int32_t pos_start, int32_t *kept_out_host, void *cuda_stream);
+
+/* Fills *out for (stream, layer).  No synchronisation.                                               */
+int hermes_get_cache(hermes_t *h, int32_t stream, int32_t layer, hermes_cache_view *out);
+
+/* Host-tracked token count per layer (same for every stream and layer).                              */
+int32_t hermes_len(const hermes_t *h);
+
+/* Device-side sticky status word, read with a blocking copy: 0 = ok; bit0 = M-RoPE coordinate range
+ * too wide to compact, bit1 = rotary delta outside the table (slow path taken; results still valid).  */
+int hermes_device_status(hermes_t *h, int32_t *status_out);
+
+/* Per-kernel timing: when enabled, CUDA events bracket each kernel of the next append calls.
+ * hermes_get_profile() synchronises on the last call's events and writes up to n kernel durations in
+ * milliseconds, in HERMES_K_* order (0 for kernels that did not run); returns the count written.      */
+enum { HERMES_K_APPEND = 0, HERMES_K_SCORE_STATS = 1, HERMES_K_SCORE_COMBINE = 2,
+       HERMES_K_SCORE_COLSUM = 3, HERMES_K_SELECT = 4, HERMES_K_GATHER = 5, HERMES_K_COUNT = 6 };
+int hermes_set_profiling(hermes_t *h, int32_t enable);
+int hermes_get_profile(hermes_t *h, float *ms_out, int32_t n);
+
+/* Which scoring path the last eviction used: HERMES_SCORE_SIMT or HERMES_SCORE_TCGEN05 (0 if none).  */
+int32_t hermes_last_score_path(const hermes_t *h);
+
+/* Number of kernels launched by the last append call.                                                */
+int32_t hermes_last_launch_count(const hermes_t *h);
+
+void hermes_destroy(hermes_t *h);
+
+/* Message of the last failing call on this handle (or of the last failing hermes_create if h == NULL). */
+const char *hermes_last_error(const hermes_t *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HERMES_H_ */

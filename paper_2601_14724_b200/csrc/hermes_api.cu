@@ -1,0 +1,344 @@
+// C-ABI entry points (include/hermes.h): config validation, workspace carve-up, and the stream-ordered
+// launch sequence of one chunk arrival.  No host synchronisation on the success path of an append.
+#include <climits>
+
+#include "host_state.cuh"
+#include "k_append.cuh"
+#include "k_gather.cuh"
+#include "k_score_simt.cuh"
+#include "k_select.cuh"
+#include "k_score_tc.cuh"
+
+using namespace hk;
+
+static thread_local std::string g_create_error;
+
+static int fail(hermes_t* h, int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  if (h) h->err = buf; else g_create_error = buf;
+  return code;
+}
+
+#define CUDA_TRY(h, call)                                                                     \
+  do {                                                                                        \
+    cudaError_t e_ = (call);                                                                  \
+    if (e_ != cudaSuccess) return fail(h, HERMES_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+  } while (0)
+
+extern "C" void hermes_default_config(hermes_config* c) {
+  if (!c) return;
+  memset(c, 0, sizeof *c);
+  c->n_streams = 1;
+  c->dtype = HERMES_BF16;
+  c->n_shallow = c->n_deep = c->l_short = c->l_long = -1;
+  c->omega0 = 0.75f; c->gamma = 0.6f;
+  c->lambda_shallow = 0.1f; c->lambda_middle = 0.3f; c->lambda_deep = 0.4f;
+  c->norm_mode = HERMES_NORM_MAX;
+  c->rope_mode = HERMES_ROPE_1D; c->rope_theta = 10000.f;
+  c->mrope_section[0] = 16; c->mrope_section[1] = 24; c->mrope_section[2] = 24;
+  c->mrope_compact_axes = 1; c->mrope_grid_h = 8; c->mrope_grid_w = 8;
+  c->max_probe_tokens = 64;
+  c->score_path = HERMES_SCORE_AUTO;
+}
+
+extern "C" size_t hermes_workspace_bytes(const hermes_config* c) {
+  if (!c || validate(*c)) return 0;
+  return make_layout(*c).total;
+}
+
+extern "C" const char* hermes_last_error(const hermes_t* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+extern "C" int32_t hermes_len(const hermes_t* h) { return h ? h->len : 0; }
+extern "C" int32_t hermes_last_score_path(const hermes_t* h) { return h ? h->last_score_path : 0; }
+extern "C" int32_t hermes_last_launch_count(const hermes_t* h) { return h ? h->last_launches : 0; }
+
+extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t bytes, hermes_t** out) {
+  if (out) *out = nullptr;
+  if (!c || !out) return fail(nullptr, HERMES_EINVAL, "null argument");
+  if (const char* why = validate(*c)) return fail(nullptr, HERMES_EINVAL, "%s", why);
+  const Layout y = make_layout(*c);
+  if (!workspace) return fail(nullptr, HERMES_EINVAL, "null workspace");
+  if (reinterpret_cast<uintptr_t>(workspace) % 256) return fail(nullptr, HERMES_EINVAL, "workspace must be 256-byte aligned");
+  if (bytes < y.total) return fail(nullptr, HERMES_ECAPACITY, "workspace of %zu bytes < %zu needed", bytes, y.total);
+
+  int n_dev = 0;
+  if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev <= 0 || c->device < 0 || c->device >= n_dev) {
+    (void)cudaGetLastError();
+    return fail(nullptr, HERMES_ECUDA, "no usable CUDA device %d (found %d): this library has no CPU fallback", c->device, n_dev);
+  }
+  cudaDeviceProp prop;
+  CUDA_TRY(nullptr, cudaGetDeviceProperties(&prop, c->device));
+  if (prop.major != 10) return fail(nullptr, HERMES_ECUDA, "device %d is sm_%d%d; kernels are built for sm_100a only", c->device, prop.major, prop.minor);
+  if (size_t(y.cap) * 4 + 24 * 1024 > prop.sharedMemPerBlockOptin)
+    return fail(nullptr, HERMES_EINVAL, "max_tokens %d too large for the select kernel's shared memory", y.cap);
+  CUDA_TRY(nullptr, cudaSetDevice(c->device));
+
+  hermes_t* h = new (std::nothrow) hermes;
+  if (!h) return fail(nullptr, HERMES_ENOMEM, "out of host memory");
+  h->cfg = *c; h->lay = y; h->ws = static_cast<char*>(workspace);
+  h->next_pos = c->pos_offset;
+
+  Geom& g = h->geom;
+  g.B = c->n_streams; g.L = c->n_layers; g.Hq = c->n_q_heads; g.Hkv = c->n_kv_heads;
+  g.G = c->n_q_heads / c->n_kv_heads; g.d = c->head_dim;
+  g.cap = y.cap; g.budget = c->budget; g.n_axes = y.n_axes; g.row_elems = c->n_kv_heads * c->head_dim;
+  g.n_shallow = y.n_shallow; g.p_max = c->max_probe_tokens; g.pos_offset = c->pos_offset;
+  g.sec_t = c->mrope_section[0]; g.sec_h = c->mrope_section[1];
+  g.compact_axes = c->mrope_compact_axes; g.grid_h = c->mrope_grid_h; g.grid_w = c->mrope_grid_w;
+  g.table_rows = y.table_rows;
+  g.kc = h->ws + y.kc; g.vc = h->ws + y.vc; g.posc = reinterpret_cast<int32_t*>(h->ws + y.posc);
+  g.colsum = reinterpret_cast<float*>(h->ws + y.colsum);
+  g.rowstat = reinterpret_cast<float*>(h->ws + y.rowstat);
+  g.partial = reinterpret_cast<float*>(h->ws + y.partial);
+  g.scores = reinterpret_cast<float*>(h->ws + y.scores);
+  g.kept = reinterpret_cast<int32_t*>(h->ws + y.kept);
+  g.rope_tab = reinterpret_cast<float2*>(h->ws + y.rope_tab);
+  g.rope_freq = reinterpret_cast<double*>(h->ws + y.rope_freq);
+  g.omega = reinterpret_cast<float*>(h->ws + y.omega);
+  g.lambda = reinterpret_cast<float*>(h->ws + y.lambda);
+  g.status = reinterpret_cast<int32_t*>(h->ws + y.status);
+
+  // per-layer recency weight (Eq. 3-4) and smoothing weight (Eq. 7)
+  const int L = c->n_layers, ns = y.n_shallow, nm = y.n_middle;
+  const int l_short = c->l_short >= 0 ? c->l_short : ns;
+  const int l_long = c->l_long >= 0 ? c->l_long : ns + nm - 1;
+  std::vector<float> omega(L), lambda(L);
+  for (int l = 0; l < L; ++l) {
+    if (l < ns) { omega[l] = 1.f; lambda[l] = c->lambda_shallow; }
+    else if (l < ns + nm) {
+      omega[l] = l_long == l_short ? c->omega0
+                                   : float(double(c->omega0) - double(c->gamma) * double(l - l_short) / double(l_long - l_short));
+      lambda[l] = c->lambda_middle;
+    } else { omega[l] = 0.f; lambda[l] = c->lambda_deep; }
+  }
+  // rotary angle table in fp64: row r holds (cos, sin)(delta * theta_j) for delta = -r
+  const int half = c->head_dim / 2;
+  std::vector<double> freq(half);
+  for (int j = 0; j < half; ++j) freq[j] = std::pow(double(c->rope_theta), -2.0 * double(j) / double(c->head_dim));
+  std::vector<float2> tab(size_t(y.table_rows) * half);
+  for (int r = 0; r < y.table_rows; ++r)
+    for (int j = 0; j < half; ++j) {
+      const double ang = double(-r) * freq[j];
+      tab[size_t(r) * half + j] = make_float2(float(std::cos(ang)), float(std::sin(ang)));
+    }
+  cudaError_t e = cudaSuccess;
+  auto up = [&](void* dst, const void* src, size_t n) { if (e == cudaSuccess) e = cudaMemcpy(dst, src, n, cudaMemcpyHostToDevice); };
+  up(g.omega, omega.data(), L * 4); up(g.lambda, lambda.data(), L * 4);
+  up(g.rope_freq, freq.data(), half * 8); up(g.rope_tab, tab.data(), tab.size() * 8);
+  if (e == cudaSuccess) e = cudaMemset(g.status, 0, 256);
+  if (e == cudaSuccess) e = cudaMemset(g.posc, 0, size_t(g.B) * L * 2 * y.n_axes * y.cap * 4);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_select, cudaFuncAttributeMaxDynamicSharedMemorySize, y.cap * 4);
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  if (e != cudaSuccess) {
+    fail(nullptr, HERMES_ECUDA, "create: %s", cudaGetErrorString(e));
+    delete h;
+    return HERMES_ECUDA;
+  }
+  // tensor-core scoring path: bf16, d = 128; probing it builds its tensor maps
+  h->tc_ok = tc_init(h);
+  if (c->score_path == HERMES_SCORE_TCGEN05 && !h->tc_ok) {
+    std::string why = h->err;
+    delete h;
+    return fail(nullptr, HERMES_EINVAL, "tcgen05 scoring path unavailable for this config: %s", why.c_str());
+  }
+  *out = h;
+  return HERMES_OK;
+}
+
+extern "C" void hermes_destroy(hermes_t* h) {
+  if (!h) return;
+  if (h->timer.created)
+    for (int i = 0; i < HERMES_K_COUNT; ++i) { cudaEventDestroy(h->timer.beg[i]); cudaEventDestroy(h->timer.end[i]); }
+  tc_destroy(h);
+  delete h;
+}
+
+extern "C" int hermes_set_profiling(hermes_t* h, int32_t enable) {
+  if (!h) return HERMES_EINVAL;
+  if (enable && !h->timer.created) {
+    for (int i = 0; i < HERMES_K_COUNT; ++i) {
+      CUDA_TRY(h, cudaEventCreate(&h->timer.beg[i]));
+      CUDA_TRY(h, cudaEventCreate(&h->timer.end[i]));
+    }
+    h->timer.created = true;
+  }
+  h->profiling = enable != 0;
+  return HERMES_OK;
+}
+
+extern "C" int hermes_get_profile(hermes_t* h, float* ms_out, int32_t n) {
+  if (!h || !ms_out || n < 0) return HERMES_EINVAL;
+  if (!h->timer.created) return fail(h, HERMES_ESTATE, "profiling was never enabled");
+  int w = 0;
+  for (; w < n && w < HERMES_K_COUNT; ++w) {
+    ms_out[w] = 0.f;
+    if (!h->timer.ran[w]) continue;
+    CUDA_TRY(h, cudaEventSynchronize(h->timer.end[w]));
+    CUDA_TRY(h, cudaEventElapsedTime(&ms_out[w], h->timer.beg[w], h->timer.end[w]));
+  }
+  return w;
+}
+
+extern "C" int hermes_device_status(hermes_t* h, int32_t* status_out) {
+  if (!h || !status_out) return HERMES_EINVAL;
+  CUDA_TRY(h, cudaMemcpy(status_out, h->geom.status, 4, cudaMemcpyDeviceToHost));
+  return HERMES_OK;
+}
+
+extern "C" int hermes_get_cache(hermes_t* h, int32_t stream, int32_t layer, hermes_cache_view* out) {
+  if (!h || !out) return HERMES_EINVAL;
+  if (stream < 0 || stream >= h->cfg.n_streams || layer < 0 || layer >= h->cfg.n_layers)
+    return fail(h, HERMES_EINVAL, "stream %d / layer %d out of range", stream, layer);
+  const Geom& g = h->geom;
+  const size_t bl = size_t(stream) * g.L + layer, slab = bl * 2 + h->cur;
+  out->k = static_cast<char*>(g.kc) + slab * g.cap * h->lay.row_bytes;
+  out->v = static_cast<char*>(g.vc) + slab * g.cap * h->lay.row_bytes;
+  out->pos = g.posc + slab * g.n_axes * g.cap;
+  out->n_axes = g.n_axes; out->pos_stride = g.cap; out->len = h->len;
+  out->last_T = h->last_T;
+  out->last_scores = h->last_T ? g.scores + bl * g.cap : nullptr;
+  out->last_kept = h->last_T ? g.kept + bl * g.budget : nullptr;
+  return HERMES_OK;
+}
+
+namespace {
+struct Prof {                               // brackets one kernel with events when profiling is on
+  hermes_t* h; int id; cudaStream_t s;
+  Prof(hermes_t* h_, int id_, cudaStream_t s_) : h(h_), id(id_), s(s_) {
+    if (h->profiling) { cudaEventRecord(h->timer.beg[id], s); h->timer.ran[id] = true; }
+    ++h->last_launches;
+  }
+  ~Prof() { if (h->profiling) cudaEventRecord(h->timer.end[id], s); }
+};
+
+template <typename T>
+void launch_simt(hermes_t* h, const void* q, int Tn, int P, float scale_log2, cudaStream_t s) {
+  const Geom& g = h->geom;
+  const int n_part = (Tn + kSimtTokens - 1) / kSimtTokens;
+  const dim3 grid(n_part, g.Hkv, g.B * (g.L - g.n_shallow));
+  const T* qp = static_cast<const T*>(q);
+  auto run = [&](auto dconst) {
+    constexpr int D = decltype(dconst)::value;
+    { Prof p(h, HERMES_K_SCORE_STATS, s);
+      k_score_simt<T, D, false><<<grid, kSimtTokens, 0, s>>>(g, qp, h->cur, Tn, P, scale_log2, n_part); }
+    { Prof p(h, HERMES_K_SCORE_COMBINE, s);
+      const int warps = g.B * (g.L - g.n_shallow) * g.Hq * P;
+      k_score_combine<<<(warps + 7) / 8, 256, 0, s>>>(g, P, n_part); }
+    { Prof p(h, HERMES_K_SCORE_COLSUM, s);
+      k_score_simt<T, D, true><<<grid, kSimtTokens, 0, s>>>(g, qp, h->cur, Tn, P, scale_log2, n_part); }
+  };
+  if (g.d == 32) run(std::integral_constant<int, 32>{});
+  else if (g.d == 64) run(std::integral_constant<int, 64>{});
+  else run(std::integral_constant<int, 128>{});
+}
+}  // namespace
+
+extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V_new, const void* Q_probe,
+                                   int32_t n_new, int32_t n_probe, int32_t pos_start, void* cuda_stream) {
+  if (!h) return HERMES_EINVAL;
+  const hermes_config& c = h->cfg;
+  Geom& g = h->geom;
+  if (!K_new || !V_new) return fail(h, HERMES_EINVAL, "K_new / V_new must not be NULL");
+  if (n_new <= 0) return fail(h, HERMES_EINVAL, "n_new = %d must be positive", n_new);
+  if (Q_probe && (n_probe <= 0 || n_probe > c.max_probe_tokens)) return fail(h, HERMES_EINVAL, "n_probe = %d not in [1, %d]", n_probe, c.max_probe_tokens);
+  const int Tn = h->len + n_new;
+  if (Tn > g.cap) return fail(h, HERMES_ECAPACITY, "len %d + n_new %d exceeds max_tokens %d", h->len, n_new, g.cap);
+  // arrival positions (DESIGN c16): host-computable, strictly above every cached position
+  long long p0;
+  long long steps = 0;
+  if (g.n_axes == 1) {
+    p0 = pos_start >= 0 ? pos_start : c.pos_offset + h->len;
+  } else {
+    const int tpt = c.mrope_grid_h * c.mrope_grid_w;
+    steps = (n_new + tpt - 1) / tpt;
+    p0 = pos_start >= 0 ? pos_start : c.pos_offset + std::min<long long>(h->t_steps_seen, c.budget);
+  }
+  if (p0 < h->next_pos) return fail(h, HERMES_EINVAL, "pos_start %lld is not above the cached positions (need >= %lld)", p0, h->next_pos);
+  if (p0 + std::max<long long>(n_new, steps) >= INT_MAX) return fail(h, HERMES_EINVAL, "position overflow");
+  const bool evict = Q_probe != nullptr && Tn > c.budget;
+
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  h->last_launches = 0;
+  for (bool& r : h->timer.ran) r = false;
+  const int row_vecs = int(h->lay.row_bytes / 16);
+  const int BL = g.B * g.L;
+  {
+    Prof p(h, HERMES_K_APPEND, s);
+    const size_t n_vec = size_t(n_new) * row_vecs;
+    const int gx = int(std::min<size_t>((n_vec + 511) / 512, 64));
+    k_append<<<dim3(std::max(gx, 1), BL), 256, 0, s>>>(g, static_cast<const uint4*>(K_new), static_cast<const uint4*>(V_new),
+                                                      h->cur, h->len, n_new, row_vecs, int(p0));
+  }
+  if (evict) {
+    const float scale = c.softmax_scale > 0.f ? c.softmax_scale : float(1.0 / std::sqrt(double(c.head_dim)));
+    const float scale_log2 = scale * kLog2e;
+    if (g.L > g.n_shallow) {
+      const bool use_tc = h->tc_ok && c.score_path != HERMES_SCORE_SIMT &&
+                          (c.score_path == HERMES_SCORE_TCGEN05 || tc_profitable(h, Tn, n_probe));
+      if (use_tc) {
+        if (int rc = tc_score(h, Q_probe, Tn, n_probe, scale_log2, s)) return rc;
+        h->last_score_path = HERMES_SCORE_TCGEN05;
+      } else {
+        if (c.dtype == HERMES_BF16) launch_simt<__nv_bfloat16>(h, Q_probe, Tn, n_probe, scale_log2, s);
+        else launch_simt<float>(h, Q_probe, Tn, n_probe, scale_log2, s);
+        h->last_score_path = HERMES_SCORE_SIMT;
+      }
+    }
+    {
+      Prof p(h, HERMES_K_SELECT, s);
+      const double k = c.forget_rate;
+      const float r_norm_sum = float((1.0 - std::exp(-k)) / (1.0 - std::exp(-k * Tn)));
+      k_select<<<BL, kSelThreads, size_t(Tn) * 4, s>>>(g, h->cur, Tn, n_probe, c.forget_rate, c.norm_mode == HERMES_NORM_SUM, r_norm_sum);
+    }
+    {
+      Prof p(h, HERMES_K_GATHER, s);
+      const int V = c.dtype == HERMES_BF16 ? 8 : 4;
+      const int upr = g.Hkv * (g.d / 2 / V);
+      const int total = g.budget * upr;
+      const int gx = std::max(1, (total + 2 * kGatherThreads - 1) / (2 * kGatherThreads));
+      if (c.dtype == HERMES_BF16) k_gather<__nv_bfloat16><<<dim3(gx, BL), kGatherThreads, 0, s>>>(g, h->cur);
+      else k_gather<float><<<dim3(gx, BL), kGatherThreads, 0, s>>>(g, h->cur);
+    }
+  }
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(h, HERMES_ECUDA, "kernel launch failed: %s", cudaGetErrorString(e));
+  // commit host-tracked state
+  if (g.n_axes == 3) h->t_steps_seen += steps;
+  if (evict) {
+    h->cur ^= 1; h->len = c.budget; h->last_T = Tn;
+    // after eager re-indexing every cached position is below offset + budget (1D) or below
+    // offset + min(temporal steps seen, budget) (M-RoPE: a layer holds at most that many distinct t)
+    h->next_pos = c.pos_offset + (g.n_axes == 1 ? (long long)c.budget : std::min<long long>(h->t_steps_seen, c.budget));
+  } else {
+    h->len = Tn;
+    h->next_pos = p0 + (g.n_axes == 1 ? n_new : steps);
+  }
+  return HERMES_OK;
+}
+
+extern "C" int hermes_append_chunk_host(hermes_t* h, const void* K_host, const void* V_host, const void* Q_host,
+                                        int32_t n_new, int32_t n_probe, int32_t pos_start,
+                                        int32_t* kept_out_host, void* cuda_stream) {
+  if (!h) return HERMES_EINVAL;
+  if (!K_host || !V_host) return fail(h, HERMES_EINVAL, "K_new / V_new must not be NULL");
+  const hermes_config& c = h->cfg;
+  if (n_new <= 0 || n_new > c.max_chunk_tokens) return fail(h, HERMES_EINVAL, "n_new = %d not in [1, %d] (host path)", n_new, c.max_chunk_tokens);
+  if (Q_host && (n_probe <= 0 || n_probe > c.max_probe_tokens)) return fail(h, HERMES_EINVAL, "n_probe = %d not in [1, %d]", n_probe, c.max_probe_tokens);
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  const size_t BL = size_t(c.n_streams) * c.n_layers;
+  const size_t kv_bytes = BL * n_new * h->lay.row_bytes;
+  char* sk = h->ws + h->lay.stage_k; char* sv = h->ws + h->lay.stage_v; char* sq = h->ws + h->lay.stage_q;
+  CUDA_TRY(h, cudaMemcpyAsync(sk, K_host, kv_bytes, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(h, cudaMemcpyAsync(sv, V_host, kv_bytes, cudaMemcpyHostToDevice, s));
+  if (Q_host) CUDA_TRY(h, cudaMemcpyAsync(sq, Q_host, BL * c.n_q_heads * n_probe * c.head_dim * h->lay.esize, cudaMemcpyHostToDevice, s));
+  const int len_before = h->len;
+  int rc = hermes_append_chunk(h, sk, sv, Q_host ? sq : nullptr, n_new, n_probe, pos_start, cuda_stream);
+  if (rc != HERMES_OK) return rc;
+  const bool evicted = Q_host && len_before + n_new > c.budget;
+  if (kept_out_host && evicted)
+    CUDA_TRY(h, cudaMemcpyAsync(kept_out_host, h->geom.kept, BL * c.budget * 4, cudaMemcpyDeviceToHost, s));
+  return HERMES_OK;
+}

@@ -1,0 +1,130 @@
+// Host-side state of a handle: validated config, workspace carve-up, host-tracked stream state.
+#pragma once
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/hermes.h"
+#include "common.cuh"
+
+namespace hk {
+
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+struct Layout {           // byte offsets into the workspace
+  size_t kc, vc, posc, colsum, rowstat, partial, scores, kept, rope_tab, rope_freq, omega, lambda,
+      status, stage_k, stage_v, stage_q, tmaps, total;
+  int cap, n_axes, n_part_max, table_rows, n_shallow, n_middle, n_deep;
+  size_t esize, row_bytes;
+};
+
+inline void stage_split(int L, int& n_shallow, int& n_deep) {   // PAPER.md:144; rounding DESIGN c7
+  if (n_shallow < 0) n_shallow = std::max(1, (L + 5) / 10);
+  if (n_deep < 0) n_deep = std::max(1, (3 * L + 5) / 10);
+}
+
+// Returns nullptr if valid, else a static message.
+inline const char* validate(const hermes_config& c) {
+  if (c.n_layers <= 0 || c.n_layers > kMaxLayers) return "n_layers out of range [1, 256]";
+  if (c.n_q_heads <= 0 || c.n_kv_heads <= 0 || c.n_q_heads % c.n_kv_heads) return "n_q_heads must be a positive multiple of n_kv_heads";
+  if (c.head_dim != 32 && c.head_dim != 64 && c.head_dim != 128) return "head_dim must be 32, 64 or 128";
+  if (c.dtype != HERMES_F32 && c.dtype != HERMES_BF16) return "dtype must be HERMES_F32 or HERMES_BF16";
+  if (c.n_streams <= 0) return "n_streams must be positive";
+  if (c.budget <= 0) return "budget must be positive";
+  if (c.max_chunk_tokens <= 0) return "max_chunk_tokens must be positive";
+  if (c.max_probe_tokens <= 0) return "max_probe_tokens must be positive";
+  if (c.max_tokens != 0 && c.max_tokens <= c.budget) return "max_tokens must exceed budget (or be 0)";
+  if (!(c.forget_rate > 0.f) || !std::isfinite(c.forget_rate)) return "forget_rate (k of Eq. 1) must be > 0";
+  if (c.norm_mode != HERMES_NORM_MAX && c.norm_mode != HERMES_NORM_SUM) return "bad norm_mode";
+  int ns = c.n_shallow, nd = c.n_deep;
+  stage_split(c.n_layers, ns, nd);
+  if (ns < 0 || nd < 0 || ns + nd > c.n_layers) return "n_shallow + n_deep exceeds n_layers";
+  if (c.l_short >= 0 && c.l_long >= 0 && c.l_long < c.l_short) return "l_long < l_short";
+  const float lam[3] = {c.lambda_shallow, c.lambda_middle, c.lambda_deep};
+  for (float v : lam) if (!(v >= 0.f && v <= 1.f)) return "lambda must lie in [0, 1]";
+  if (c.softmax_scale < 0.f || !std::isfinite(c.softmax_scale)) return "softmax_scale must be >= 0";
+  if (c.rope_mode != HERMES_ROPE_1D && c.rope_mode != HERMES_ROPE_M3D) return "bad rope_mode";
+  if (!(c.rope_theta > 0.f)) return "rope_theta must be > 0";
+  if (c.rope_mode == HERMES_ROPE_M3D) {
+    if (c.mrope_section[0] < 0 || c.mrope_section[1] < 0 || c.mrope_section[2] < 0 ||
+        c.mrope_section[0] + c.mrope_section[1] + c.mrope_section[2] != c.head_dim / 2)
+      return "mrope_section must sum to head_dim/2";
+    if (c.mrope_grid_h <= 0 || c.mrope_grid_w <= 0) return "mrope grid must be positive";
+    if (c.mrope_compact_axes < 0 || c.mrope_compact_axes > 7) return "bad mrope_compact_axes";
+  }
+  if (c.pos_offset < 0) return "pos_offset must be >= 0";
+  if (c.score_path < HERMES_SCORE_AUTO || c.score_path > HERMES_SCORE_TCGEN05) return "bad score_path";
+  if (size_t(c.budget) + size_t(c.max_chunk_tokens) > (size_t(1) << 24)) return "budget + chunk too large";
+  return nullptr;
+}
+
+inline Layout make_layout(const hermes_config& c) {
+  Layout y{};
+  y.cap = c.max_tokens ? c.max_tokens : c.budget + c.max_chunk_tokens;
+  y.n_axes = c.rope_mode == HERMES_ROPE_M3D ? 3 : 1;
+  y.esize = c.dtype == HERMES_BF16 ? 2 : 4;
+  y.row_bytes = size_t(c.n_kv_heads) * c.head_dim * y.esize;
+  y.n_part_max = (y.cap + 127) / 128;
+  int ns = c.n_shallow, nd = c.n_deep;
+  stage_split(c.n_layers, ns, nd);
+  y.n_shallow = ns; y.n_deep = nd; y.n_middle = c.n_layers - ns - nd;
+  if (c.rope_mode == HERMES_ROPE_M3D) {
+    const int tpt = c.mrope_grid_h * c.mrope_grid_w;
+    y.table_rows = c.budget + (c.max_chunk_tokens + tpt - 1) / tpt + 2;
+  } else {
+    y.table_rows = y.cap - c.budget + 1;
+  }
+  const size_t BL = size_t(c.n_streams) * c.n_layers;
+  const size_t rows = size_t(c.n_q_heads) * c.max_probe_tokens;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+  y.kc = take(BL * 2 * y.cap * y.row_bytes);
+  y.vc = take(BL * 2 * y.cap * y.row_bytes);
+  y.posc = take(BL * 2 * y.n_axes * y.cap * 4);
+  y.colsum = take(BL * c.n_kv_heads * y.cap * 4);
+  y.rowstat = take(BL * rows * 2 * 4);
+  y.partial = take(BL * rows * y.n_part_max * 2 * 4);
+  y.scores = take(BL * y.cap * 4);
+  y.kept = take(BL * c.budget * 4);
+  y.rope_tab = take(size_t(y.table_rows) * (c.head_dim / 2) * 8);
+  y.rope_freq = take(size_t(c.head_dim / 2) * 8);
+  y.omega = take(size_t(c.n_layers) * 4);
+  y.lambda = take(size_t(c.n_layers) * 4);
+  y.status = take(256);
+  y.stage_k = take(BL * c.max_chunk_tokens * y.row_bytes);
+  y.stage_v = take(BL * c.max_chunk_tokens * y.row_bytes);
+  y.stage_q = take(BL * rows * c.head_dim * y.esize);
+  y.tmaps = take(4096);
+  y.total = o;
+  return y;
+}
+
+struct KernelTimer {
+  cudaEvent_t beg[HERMES_K_COUNT]{}, end[HERMES_K_COUNT]{};
+  bool ran[HERMES_K_COUNT]{};
+  bool created = false;
+};
+
+}  // namespace hk
+
+struct hermes {
+  hermes_config cfg{};
+  hk::Layout lay{};
+  hk::Geom geom{};
+  char* ws = nullptr;
+  int len = 0;              // tokens per layer (host-tracked; identical for all streams / layers)
+  int cur = 0;              // which half of the double buffer is current
+  long long t_steps_seen = 0;   // M-RoPE temporal steps appended so far
+  long long next_pos = 0;   // smallest admissible pos_start of the next chunk
+  int last_T = 0;
+  int last_score_path = 0;
+  int last_launches = 0;
+  bool profiling = false;
+  bool tc_ok = false;       // tcgen05 scoring path usable for this config + device
+  hk::KernelTimer timer;
+  std::string err;
+  void* tc_state = nullptr; // opaque state of the tensor-core scoring path (tensor maps, ...)
+};

@@ -1,0 +1,174 @@
+"""Lock-step parity driver: before each checked update the GPU state is downloaded through
+hermes_get_cache, handed together with the same chunk / probe to the CPU oracle, the GPU update runs
+through the C ABI, and the single-step outputs are compared.
+
+Tolerances (BASELINE.json north_star):
+  kept index sets  bit-exact, except tokens whose ORACLE score is within 1e-4 relative of the k-th threshold
+  gathered V       bit-exact
+  re-indexed K     1e-5 relative of the rotary pair's norm (fp32) / max(2 bf16 ulp, that) (bf16)  [DESIGN c15]
+  scores           1e-3 relative
+  positions        exact
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+import paper_2601_14724_b200 as hb
+from helpers import Feeder, bf16_ulp, fill_chunks, oracle_config
+from oracle import hermes_oracle as ho
+
+SCORE_RTOL = 1e-3
+BAND_RTOL = 1e-4
+K_RTOL = 1e-5
+
+
+def to_dev(x: np.ndarray, dtype: str):
+    t = torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    return t.to(torch.bfloat16) if dtype == "bf16" else t
+
+
+class LockStep:
+    def __init__(self, wl, cfg_over=None, oracle_over=None, streams=None):
+        self.wl = wl
+        self.B = wl.n_streams
+        self.cfg = hb.config_for_workload(wl, **(cfg_over or {}))
+        self.h = hb.hermes_create(self.cfg)
+        self.ocfg = oracle_config(wl, **(oracle_over or {}))
+        self.feeders = [Feeder(wl, b) for b in range(self.B)]
+        self.checked_streams = list(range(self.B)) if streams is None else streams
+        self.t_steps_seen = 0
+        self.ids = [np.zeros((wl.n_layers, 0), np.int64) for _ in range(self.B)]
+        self.report = []
+
+    def close(self):
+        hb.hermes_destroy(self.h)
+
+    # ---- state transfer -------------------------------------------------------------------------
+    def gpu_state(self, b: int) -> ho.OracleStream:
+        """Oracle stream initialised with the GPU's current cache of stream b."""
+        torch.cuda.synchronize()
+        wl = self.wl
+        st = ho.OracleStream(self.ocfg)
+        n = hb.hermes_len(self.h)
+        st._ensure(max(n, 1))
+        for l in range(wl.n_layers):
+            v = hb.hermes_get_cache(self.h, b, l)
+            st.K[l, :n] = v["k"].float().cpu().numpy()
+            st.V[l, :n] = v["v"].float().cpu().numpy()
+            st.pos[l, :, :n] = v["pos"].cpu().numpy()
+        st.len = n
+        st.t_steps_seen = self.t_steps_seen
+        return st
+
+    def _arrival(self, n_new, pos_start=-1):
+        st = ho.OracleStream(self.ocfg)
+        st.len = hb.hermes_len(self.h)
+        st.t_steps_seen = self.t_steps_seen
+        return ho.arrival_positions(self.ocfg, st, n_new, pos_start)
+
+    def _gen(self, n_new, with_probe, n_probe=None, pos_start=-1):
+        ap = self._arrival(n_new, pos_start)
+        per = [fd.next(n_new, ap, with_probe, n_probe) for fd in self.feeders]
+        K = np.stack([p[0] for p in per]); V = np.stack([p[1] for p in per])
+        Q = np.stack([p[2] for p in per]) if with_probe else None
+        return K, V, Q, [p[3] for p in per]
+
+    def _after(self, n_new, new_ids, evicted):
+        if self.ocfg.rope_mode == "m3d":
+            tpt = self.ocfg.mrope_grid_h * self.ocfg.mrope_grid_w
+            self.t_steps_seen += (n_new + tpt - 1) // tpt
+        for b in range(self.B):
+            self.ids[b] = np.concatenate([self.ids[b], np.broadcast_to(new_ids[b], (self.wl.n_layers, n_new))], 1)
+        if evicted:
+            torch.cuda.synchronize()
+            for b in range(self.B):
+                kept = np.stack([hb.hermes_get_cache(self.h, b, l)["last_kept"].cpu().numpy()
+                                 for l in range(self.wl.n_layers)]).astype(np.int64)
+                self.ids[b] = np.take_along_axis(self.ids[b], kept, axis=1)
+
+    # ---- schedule -------------------------------------------------------------------------------
+    def fill(self):
+        for n in fill_chunks(self.wl):
+            K, V, _, ids = self._gen(n, False)
+            hb.hermes_append_chunk(self.h, to_dev(K, self.wl.dtype), to_dev(V, self.wl.dtype), None)
+            self._after(n, ids, False)
+
+    def step(self, check=True, n_new=None, n_probe=None, pos_start=-1):
+        wl = self.wl
+        n_new = wl.chunk_tokens if n_new is None else n_new
+        K, V, Q, ids = self._gen(n_new, True, n_probe, pos_start)
+        pre = {b: self.gpu_state(b) for b in self.checked_streams} if check else {}
+        T = hb.hermes_len(self.h) + n_new
+        hb.hermes_append_chunk(self.h, to_dev(K, wl.dtype), to_dev(V, wl.dtype), to_dev(Q, wl.dtype), pos_start)
+        torch.cuda.synchronize()
+        evicted = T > wl.budget
+        self._after(n_new, ids, evicted)
+        results = []
+        for b, st in pre.items():
+            out = ho.oracle_step(st, K[b], V[b], Q[b], pos_start)
+            assert out["evicted"] == evicted
+            results.append(self.compare(b, st, out) if evicted else self.compare_append(b, st))
+        return results
+
+    # ---- comparisons ----------------------------------------------------------------------------
+    def compare_append(self, b, st):
+        for l in range(self.wl.n_layers):
+            v = hb.hermes_get_cache(self.h, b, l)
+            n = st.len
+            assert v["len"] == n
+            assert np.array_equal(v["k"].float().cpu().numpy(), st.K[l, :n])
+            assert np.array_equal(v["v"].float().cpu().numpy(), st.V[l, :n])
+            assert np.array_equal(v["pos"].cpu().numpy(), st.pos[l, :, :n])
+        return {"evicted": False}
+
+    def compare(self, b, st, out):
+        wl, M = self.wl, self.wl.budget
+        half = wl.head_dim // 2
+        rep = dict(stream=b, T=out["T"], band_layers=0, band_tokens=0, max_score_rel=0.0, k_mismatch_bits=0,
+                   k_max_err_norm=0.0)
+        for l in range(wl.n_layers):
+            v = hb.hermes_get_cache(self.h, b, l)
+            assert v["len"] == M and v["last_T"] == out["T"]
+            s_gpu = v["last_scores"].cpu().numpy().astype(np.float64)
+            s_or = out["S_tilde"][l]
+            rel = np.abs(s_gpu - s_or) / np.maximum(np.abs(s_or), 1e-30)
+            ok = (rel <= SCORE_RTOL) | (np.abs(s_gpu - s_or) <= 1e-37)
+            assert ok.all(), f"layer {l}: score rel err {rel.max():.3e} at {rel.argmax()}"
+            rep["max_score_rel"] = max(rep["max_score_rel"], float(rel.max()))
+            kept_gpu = v["last_kept"].cpu().numpy().astype(np.int64)
+            kept_or = out["kept"][l]
+            assert len(kept_gpu) == M and (np.diff(kept_gpu) > 0).all() and kept_gpu[0] >= 0 and kept_gpu[-1] < out["T"]
+            same = np.array_equal(kept_gpu, kept_or)
+            if not same:
+                tau = s_or[kept_or].min()
+                diff = np.setxor1d(kept_gpu, kept_or)
+                in_band = np.abs(s_or[diff] - tau) <= BAND_RTOL * abs(tau)
+                assert in_band.all(), f"layer {l}: kept sets differ outside the near-tie band: {diff[~in_band][:8]}"
+                rep["band_layers"] += 1
+                rep["band_tokens"] += len(diff)
+            # rows both sides kept: V bit-exact, K within tolerance, positions exact when the sets agree
+            k_gpu = v["k"].float().cpu().numpy(); v_gpu = v["v"].float().cpu().numpy()
+            p_gpu = v["pos"].cpu().numpy().astype(np.int64)
+            if same:
+                sel_g = sel_o = np.arange(M)
+                assert np.array_equal(p_gpu, st.pos[l, :, :M]), f"layer {l}: positions differ"
+            else:
+                common = np.intersect1d(kept_gpu, kept_or)
+                sel_g = np.searchsorted(kept_gpu, common); sel_o = np.searchsorted(kept_or, common)
+                assert (np.diff(p_gpu[0]) >= 0).all()
+            assert np.array_equal(v_gpu[sel_g].view(np.uint32), st.V[l, :M][sel_o].view(np.uint32)), f"layer {l}: V not bit-exact"
+            if same:
+                kg, ko = k_gpu[sel_g], st.K[l, :M][sel_o]
+                rep["k_mismatch_bits"] += int((kg.view(np.uint32) != ko.view(np.uint32)).sum())
+                nrm = np.hypot(ko[..., :half].astype(np.float64), ko[..., half:].astype(np.float64))
+                nrm2 = np.concatenate([nrm, nrm], -1)
+                tol = K_RTOL * nrm2
+                if wl.dtype == "bf16":
+                    tol = np.maximum(tol, 2 * bf16_ulp(ko))
+                err = np.abs(kg.astype(np.float64) - ko)
+                assert (err <= tol + 1e-30).all(), f"layer {l}: K err {err.max():.3e} beyond tolerance"
+                rep["k_max_err_norm"] = max(rep["k_max_err_norm"], float((err / np.maximum(nrm2, 1e-30)).max()))
+        rep["evicted"] = True
+        self.report.append(rep)
+        return rep

@@ -1,0 +1,79 @@
+"""CPU-side checks of the C-ABI boundary: the library loads, exports every symbol include/hermes.h
+declares, validates configs, sizes workspaces, and fails loudly without a GPU (no compute calls)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+import torch
+
+import paper_2601_14724_b200 as hb
+from workloads import CONFIGS
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    lib = hb.load_library()
+    header = open(os.path.join(ROOT, "include", "hermes.h")).read()
+    declared = set(re.findall(r"\b(hermes_[a-z_]+)\s*\(", header))
+    declared -= {"hermes_append_chunk_"}
+    assert declared == set(hb.EXPORTS)
+    for name in declared:
+        assert getattr(lib, name) is not None
+
+
+def test_config_struct_matches_header_size():
+    # 15 int32 + 3 float + int32 + 4 float + int32 + float + 3 int32 + 6 int32 = 34 x 4 bytes
+    assert C.sizeof(hb.HermesConfig) == 34 * 4
+    cfg = hb.hermes_default_config()
+    assert (cfg.omega0, cfg.gamma) == (0.75, pytest.approx(0.6))
+    assert (cfg.lambda_shallow, cfg.lambda_middle, cfg.lambda_deep) == (pytest.approx(0.1), pytest.approx(0.3), pytest.approx(0.4))
+    assert list(cfg.mrope_section) == [16, 24, 24]
+
+
+def test_workspace_bytes_accounts_for_double_buffered_cache():
+    wl = CONFIGS["llava_ov_7b"]
+    cfg = hb.config_for_workload(wl)
+    n = hb.hermes_workspace_bytes(cfg)
+    kv = 2 * 2 * wl.n_layers * wl.cap * wl.n_kv_heads * wl.head_dim * 2      # K+V, two buffers, bf16
+    assert kv < n < kv * 1.5
+    big = hb.config_for_workload(CONFIGS["batched_72b"])
+    assert hb.hermes_workspace_bytes(big) < 120e9                              # fits one B200 (180 GB)
+
+
+@pytest.mark.parametrize("field,value", [("n_kv_heads", 3), ("head_dim", 100), ("budget", 0), ("forget_rate", 0.0),
+                                         ("n_shallow", 20), ("lambda_deep", 1.5), ("mrope_section", (16, 24, 20)),
+                                         ("dtype", 7), ("max_tokens", 10)])
+def test_invalid_configs_are_rejected(field, value):
+    over = {field: value}
+    if field == "mrope_section":
+        over["rope_mode"] = hb.HERMES_ROPE_M3D
+    if field == "n_shallow":
+        over["n_deep"] = 20
+    cfg = hb.config_for_workload(CONFIGS["llava_ov_7b"], **over)
+    assert hb.hermes_workspace_bytes(cfg) == 0
+    out = C.c_void_p()
+    rc = hb.load_library().hermes_create(C.byref(cfg), None, 0, C.byref(out))
+    assert rc == hb.HERMES_EINVAL and not out.value
+    assert hb.load_library().hermes_last_error(None)
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU failure mode")
+def test_create_without_gpu_fails_loudly():
+    cfg = hb.config_for_workload(CONFIGS["toy"])
+    with pytest.raises(hb.HermesError) as e:
+        hb.hermes_create(cfg)
+    assert e.value.code == hb.HERMES_ECUDA
+    buf = C.create_string_buffer(hb.hermes_workspace_bytes(cfg) + 512)
+    addr = (C.addressof(buf) + 255) // 256 * 256
+    out = C.c_void_p()
+    rc = hb.load_library().hermes_create(C.byref(cfg), C.c_void_p(addr), hb.hermes_workspace_bytes(cfg), C.byref(out))
+    assert rc == hb.HERMES_ECUDA and b"no CPU fallback" in hb.load_library().hermes_last_error(None)
+
+
+def test_null_handle_calls_do_not_crash():
+    lib = hb.load_library()
+    assert lib.hermes_append_chunk(None, None, None, None, 1, 0, -1, None) == hb.HERMES_EINVAL
+    assert lib.hermes_len(None) == 0
+    lib.hermes_destroy(None)

@@ -1,0 +1,177 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, lock-step, on the seeded
+workloads of BASELINE.json (`configs[0..4]`, full size where the oracle finishes in seconds)."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2601_14724_b200 as hb
+from gpu_harness import LockStep, to_dev
+from workloads import CONFIGS, rope_at_arrival, sweep_point
+
+pytestmark = pytest.mark.gpu
+
+
+def _run(wl, n_checked, n_warm=0, cfg_over=None, oracle_over=None, streams=None):
+    ls = LockStep(wl, cfg_over, oracle_over, streams)
+    try:
+        ls.fill()
+        for _ in range(n_warm):
+            ls.step(check=False)
+        reps = []
+        for _ in range(n_checked):
+            reps += ls.step(check=True)
+        assert hb.hermes_device_status(ls.h) == 0
+        return ls, reps
+    except Exception:
+        ls.close()
+        raise
+
+
+def test_toy_config_all_ten_updates():
+    """configs[0]: preload 128, ten scored arrivals (T = 160 then 128), every one checked."""
+    wl = CONFIGS["toy"]
+    ls, reps = _run(wl, 10)
+    assert [r["T"] for r in reps] == [160] + [128] * 9
+    assert hb.hermes_last_score_path(ls.h) == hb.HERMES_SCORE_SIMT        # fp32 cache -> CUDA-core path
+    # end to end on the GPU state: every retained key == RoPE(k0[id], offset + slot) (rotation composition)
+    fd = ls.feeders[0]
+    for l in range(wl.n_layers):
+        v = hb.hermes_get_cache(ls.h, 0, l)
+        k0 = np.stack([fd.k0_by_id[int(t)][l] for t in ls.ids[0][l]])[None]
+        ref = rope_at_arrival(k0, np.arange(wl.budget)[None, :], wl)[0]
+        np.testing.assert_allclose(v["k"].float().cpu().numpy(), ref, atol=2e-5)
+        assert v["pos"].cpu().numpy()[0].tolist() == list(range(wl.budget))
+    ls.close()
+
+
+def test_llava_geometry_reduced_multi_tile_ragged():
+    """LLaVA-OV-7B geometry, fewer layers / smaller budget: T = 1764 spans 13.8 token tiles."""
+    wl = CONFIGS["llava_ov_7b"].scaled(n_layers=10, budget=1568, probe_tokens=24)
+    ls, reps = _run(wl, 3, n_warm=1)
+    assert all(r["max_score_rel"] < 1e-3 for r in reps)
+    ls.close()
+
+
+def test_llava_ov_7b_full_size():
+    """configs[1] at full size, in the launch configuration bench.py times: 2 lock-step updates."""
+    wl = CONFIGS["llava_ov_7b"]
+    ls, reps = _run(wl, 2, n_warm=2)
+    assert all(r["T"] == 6468 for r in reps)
+    ls.close()
+
+
+def test_qwen25_vl_mrope_reduced_and_all_axes():
+    wl = CONFIGS["qwen25_vl_7b"].scaled(n_layers=6, budget=1024, probe_tokens=32, pos_offset=5)
+    ls, reps = _run(wl, 3, n_warm=1)
+    ls.close()
+    wl_all = wl.scaled(mrope_compact_axes=0b111)
+    ls, reps = _run(wl_all, 2)
+    ls.close()
+
+
+def test_qwen25_vl_7b_full_size():
+    """configs[2] at full size: M-RoPE, budget 8192, chunk 128, 128 probe tokens; 1 lock-step update."""
+    ls, reps = _run(CONFIGS["qwen25_vl_7b"], 1, n_warm=1)
+    assert reps[0]["T"] == 8320
+    ls.close()
+
+
+def test_sweep_corners_reduced_layers():
+    """configs[3] corners (budget 2K / P 16 and budget 4K / P 256) on 6 layers."""
+    for budget, probe in ((2048, 16), (4096, 256)):
+        wl = sweep_point(budget, probe).scaled(n_layers=6)
+        ls, _ = _run(wl, 1, n_warm=1)
+        ls.close()
+
+
+def test_batched_72b_geometry_reduced_equals_single_streams():
+    """configs[4] geometry (64 q / 8 kv heads), 3 streams x 8 layers: oracle parity per stream, and the
+    batched call equals B single-stream calls bit for bit."""
+    wl = CONFIGS["batched_72b"].scaled(n_layers=8, n_streams=3, budget=784)
+    ls, reps = _run(wl, 2, n_warm=1)
+    batched = [[{k: t.clone() for k, t in hb.hermes_get_cache(ls.h, b, l).items() if torch.is_tensor(t)}
+                for l in range(wl.n_layers)] for b in range(3)]
+    ls.close()
+    for b in (0, 2):
+        single = wl.scaled(n_streams=1)
+        one = LockStep(single)
+        one.feeders[0].stream = b                                     # same seeded inputs as stream b
+        one.fill(); one.step(check=False); one.step(check=False); one.step(check=False)
+        torch.cuda.synchronize()
+        for l in range(wl.n_layers):
+            v = hb.hermes_get_cache(one.h, 0, l)
+            for key in ("k", "v", "pos", "last_kept", "last_scores"):
+                assert torch.equal(v[key], batched[b][l][key]), (b, l, key)
+        one.close()
+
+
+def test_edge_cases_small():
+    wl = CONFIGS["toy"].scaled(preload_tokens=0, capacity=0, chunk_tokens=32)
+    # (a) below budget and without a probe nothing is evicted; (b) evicting exactly one token; (c) one probe row
+    ls = LockStep(wl)
+    ls.step(check=True, n_new=32)                 # T = 32 <= 96: append only, even with a probe
+    ls.step(check=True, n_new=32)
+    ls.step(check=True, n_new=32)                 # T = 96 == budget: still no eviction
+    assert hb.hermes_len(ls.h) == 96
+    r = ls.step(check=True, n_new=1, n_probe=1)   # T = 97: evict exactly one token, single probe row
+    assert r[0]["evicted"] and hb.hermes_len(ls.h) == 96
+    r = ls.step(check=True, n_new=32, n_probe=3)
+    # capacity: len 96 + 33 > 128
+    K = torch.zeros(1, wl.n_layers, 33, wl.n_kv_heads, wl.head_dim, device="cuda")
+    with pytest.raises(hb.HermesError) as e:
+        hb.hermes_append_chunk(ls.h, K, K, None)
+    assert e.value.code == hb.HERMES_ECAPACITY and hb.hermes_len(ls.h) == 96
+    # explicit pos_start jump: deltas leave the rotary table -> fp64 slow path, still within tolerance
+    r = ls.step(check=True, n_new=32, pos_start=5000)
+    assert hb.hermes_device_status(ls.h) & 2
+    with pytest.raises(hb.HermesError):           # positions must stay above the cache
+        ls.step(check=False, n_new=8, pos_start=3)
+    ls.close()
+
+
+@pytest.mark.parametrize("over,oover", [
+    (dict(norm_mode=hb.HERMES_NORM_SUM), dict(norm_mode="sum")),
+    (dict(lambda_shallow=0.0, lambda_middle=0.0, lambda_deep=0.0), dict(lambda_shallow=0.0, lambda_middle=0.0, lambda_deep=0.0)),
+    (dict(n_shallow=4, n_deep=0, lambda_shallow=0.0), dict(n_shallow=4, n_deep=0, lambda_shallow=0.0)),   # FIFO
+    (dict(pos_offset=13), dict(pos_offset=13)),
+    (dict(softmax_scale=0.05, omega0=0.5, gamma=0.2, forget_rate=0.3), dict(softmax_scale=0.05, omega0=0.5, gamma=0.2, forget_rate=0.3)),
+])
+def test_hyperparameter_variants(over, oover):
+    wl = CONFIGS["toy"]
+    if "pos_offset" in over:
+        wl, over, oover = wl.scaled(pos_offset=13), {}, {}
+    ls, reps = _run(wl, 3, cfg_over=over, oracle_over=oover)
+    if over.get("n_shallow") == 4:                 # pure recency everywhere: sliding window of PAPER.md:49
+        newest = np.arange(ls.feeders[0].tokens_fed - wl.budget, ls.feeders[0].tokens_fed)
+        assert (ls.ids[0] == newest[None, :]).all()
+    ls.close()
+
+
+def test_determinism_and_host_api():
+    wl = CONFIGS["llava_ov_7b"].scaled(n_layers=5, budget=784, probe_tokens=8)
+
+    def run(host: bool):
+        ls = LockStep(wl)
+        ls.fill()
+        kept = torch.zeros(1, wl.n_layers, wl.budget, dtype=torch.int32).pin_memory()
+        for _ in range(3):
+            K, V, Q, ids = ls._gen(wl.chunk_tokens, True)
+            if host:
+                args = [torch.from_numpy(x).to(torch.bfloat16).pin_memory() for x in (K, V, Q)]
+                hb.hermes_append_chunk_host(ls.h, *args, kept_out=kept)
+            else:
+                hb.hermes_append_chunk(ls.h, to_dev(K, "bf16"), to_dev(V, "bf16"), to_dev(Q, "bf16"))
+            torch.cuda.synchronize()
+        out = [{k: t.clone() for k, t in hb.hermes_get_cache(ls.h, 0, l).items() if torch.is_tensor(t)}
+               for l in range(wl.n_layers)]
+        ls.close()
+        return out, kept.clone()
+
+    a, _ = run(False)
+    b, _ = run(False)
+    c, kept = run(True)
+    for l in range(wl.n_layers):
+        for key in ("k", "v", "pos", "last_kept", "last_scores"):
+            assert torch.equal(a[l][key], b[l][key])          # same inputs -> same bits
+            assert torch.equal(a[l][key], c[l][key])          # host-buffer entry point == device entry point
+        assert torch.equal(kept[0, l].cuda(), a[l]["last_kept"])
