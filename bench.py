@@ -1,0 +1,324 @@
+#!/usr/bin/env python
+"""Benchmark of the HERMES per-chunk KV-cache update (BASELINE.json metric) on B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+A "step" is one evicting chunk arrival (all rows a0-a7 of SURVEY.md section 8a) on the LLaVA-OV-7B
+geometry of BASELINE.json configs[1].  Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from workloads import CONFIGS, chunk_kv, probe_q  # noqa: E402
+
+METRIC, UNIT = "kv_tokens_managed_per_s", "tokens/s"
+POOL = 16          # distinct pre-generated chunk/probe sets cycled through the timed region
+
+
+# ------------------------------------------------------------------------------- shared helpers
+def algorithmic_work(wl, n_streams=1):
+    """per-update algorithmic flops / bytes of the method (not of our design)."""
+    L, T, M, P = wl.n_layers, wl.budget + wl.chunk_tokens, wl.budget, wl.probe_tokens
+    n_sh = max(1, (L + 5) // 10)
+    Ls = L - n_sh
+    es = 2 if wl.dtype == "bf16" else 4
+    row = wl.n_kv_heads * wl.head_dim * es
+    flops = 2.0 * wl.n_q_heads * P * T * wl.head_dim * Ls * n_streams
+    bytes_min = n_streams * (L * (T + 3 * M) * row + Ls * wl.n_q_heads * P * wl.head_dim * es)
+    gather_bytes = n_streams * L * 4 * M * row               # kept K,V rows read + written
+    return dict(flops=flops, bytes_min=bytes_min, gather_bytes=gather_bytes, T=T, Ls=Ls)
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm=d["hbm_gbs"], tensor=d.get("bf16_tflops_sustained", d["bf16_tflops"]),
+                    tensor_burst=d["bf16_tflops"], source="measured (MEASURED_PEAKS.json)")
+    return dict(hbm=6650.0, tensor=1400.0, tensor_burst=1590.0, source="fallback (B200_PROFILING.md)")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        self.p.wait()
+        self.f.flush()
+        rows = [r.split(",") for r in open(self.f.name).read().strip().splitlines() if r.count(",") >= 6]
+        os.unlink(self.f.name)
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm = [float(r[0]) for r in rows]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[3 + i].strip().lower().startswith("active") for r in rows)]
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": float(rows[0][1]), "samples": len(rows),
+                "power_w_max": max(float(r[2]) for r in rows), "reasons": reasons}
+
+
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def max_over_ranks(ms: float, world: int, device=None) -> float:
+    """Slowest rank's time (all_reduce MAX); identity for one process."""
+    if world == 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(wl, world: int, streams_per_rank: int, ms_per_step: float) -> float:
+    """Whole-job KV tokens managed per second: all ranks' B*L*T over the slowest rank's step time."""
+    T = wl.budget + wl.chunk_tokens
+    return world * streams_per_rank * wl.n_layers * T / (ms_per_step * 1e-3)
+
+
+def make_pool(wl, rank: int, n_sets: int):
+    """Seeded chunk / probe sets [B, L, ...] as fp32 numpy (storage-representable values)."""
+    B = wl.n_streams
+    sets = []
+    for u in range(n_sets):
+        per = [chunk_kv(wl, rank * B + b, 1000 + u, (1000 + u) * wl.chunk_tokens, wl.chunk_tokens) for b in range(B)]
+        K = np.stack([p[0] for p in per]); V = np.stack([p[1] for p in per])
+        Q = np.stack([probe_q(wl, rank * B + b, 1000 + u) for b in range(B)])
+        sets.append((K, V, Q))
+    return sets
+
+
+# ------------------------------------------------------------------------------- our arm (CUDA)
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2601_14724_b200 as hb
+
+    rank, local_rank, world = dist_env()
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    wl = CONFIGS[args.workload]
+    B = wl.n_streams
+    tdt = torch.bfloat16 if wl.dtype == "bf16" else torch.float32
+    cfg = hb.config_for_workload(wl, device=local_rank)
+    h = hb.hermes_create(cfg)
+
+    host_pool = [tuple(torch.from_numpy(x).to(tdt).pin_memory() for x in s) for s in make_pool(wl, rank, POOL)]
+    dev_pool = [tuple(x.to(dev) for x in s) for s in host_pool]
+    # fill to the budget without a probe (no eviction), then W warm evicting updates
+    n_fill = wl.budget // wl.chunk_tokens
+    for i in range(n_fill):
+        K, V, _ = dev_pool[i % POOL]
+        hb.hermes_append_chunk(h, K, V, None)
+    assert hb.hermes_len(h) == wl.budget
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(n, fn):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        for i in range(n):
+            fn(i)
+        e1.record()
+        barrier()
+        return max_over_ranks(e0.elapsed_time(e1), world, dev) / n
+
+    def dev_step(i):
+        K, V, Q = dev_pool[i % POOL]
+        hb.hermes_append_chunk(h, K, V, Q)
+
+    for i in range(max(args.warmup, 3)):
+        dev_step(i)
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    ms = timed(args.steps, dev_step)
+    clocks = sampler.stop() if sampler else None
+    launches = hb.hermes_last_launch_count(h) * args.steps
+    score_path = {1: "simt", 2: "tcgen05"}.get(hb.hermes_last_score_path(h), "none")
+
+    # per-kernel durations: CUDA events recorded by the library on the launch stream, same steps
+    hb.hermes_set_profiling(h, True)
+    n_prof = min(args.steps, 32)
+    acc = {}
+    for i in range(n_prof):
+        dev_step(i)
+        for k, v in hb.hermes_get_profile(h).items():
+            acc[k] = acc.get(k, 0.0) + v / n_prof
+    hb.hermes_set_profiling(h, False)
+
+    # end to end: HOST (pinned) inputs, H2D + update + D2H of the kept index lists inside the timed region
+    kept_host = torch.zeros(B, wl.n_layers, wl.budget, dtype=torch.int32).pin_memory()
+
+    def host_step(i):
+        K, V, Q = host_pool[i % POOL]
+        hb.hermes_append_chunk_host(h, K, V, Q, kept_out=kept_host)
+        torch.cuda.current_stream().synchronize()          # the caller consumes kept_host every step
+
+    n_e2e = min(args.steps, 64)
+    for i in range(3):
+        host_step(i)
+    ms_e2e = timed(n_e2e, host_step)
+    h2d = sum(x.numel() * x.element_size() for x in host_pool[0])
+    d2h = kept_host.numel() * 4
+
+    if rank != 0:
+        hb.hermes_destroy(h)
+        return None
+    work = algorithmic_work(wl, B)
+    pk = peaks()
+    sm = clocks.get("sm_mhz") if clocks else None
+    in_step = True                                           # kernels timed inside a long step -> sustained peak
+    kern = {k: v for k, v in acc.items() if v > 0}
+    dom = max(kern, key=kern.get)
+    t_dom = kern[dom] * 1e-3
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        traffic = json.load(open(tp)).get(dom)
+    if dom == "gather" or dom == "append":
+        ach = work["gather_bytes"] / t_dom / 1e9
+        roof = dict(kernel=dom, bound="hbm", achieved=ach, peak=pk["hbm"], unit="GB/s", frac=ach / pk["hbm"], traffic=traffic)
+    elif dom in ("score_stats", "score_colsum"):
+        ach = work["flops"] / t_dom / 1e12
+        peak = pk["tensor"] if in_step else pk["tensor_burst"]
+        roof = dict(kernel=dom, bound="tensor", achieved=ach, peak=peak, unit="TFLOP/s", frac=ach / peak, traffic=traffic)
+    else:
+        ach = wl.n_layers * B * work["T"] * 4 * 3 / t_dom / 1e9
+        roof = dict(kernel=dom, bound="hbm", achieved=ach, peak=pk["hbm"], unit="GB/s", frac=ach / pk["hbm"], traffic=traffic)
+    roof["peak_source"] = pk["source"]
+    t_roof = max(work["bytes_min"] / (pk["hbm"] * 1e9), work["flops"] / (pk["tensor"] * 1e12))
+    step_roof = dict(bound="hbm" if work["bytes_min"] / (pk["hbm"] * 1e9) >= work["flops"] / (pk["tensor"] * 1e12) else "tensor",
+                     roofline_us=t_roof * 1e6, measured_us=ms * 1e3, frac=t_roof / (ms * 1e-3),
+                     bytes_min=work["bytes_min"], flops=work["flops"])
+    out = {
+        "metric": METRIC, "value": job_value(wl, world, B, ms), "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "chunk_update_latency_us": ms * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": wl.dtype, "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[1] {wl.name}: L{wl.n_layers} Hq{wl.n_q_heads}/Hkv{wl.n_kv_heads} "
+                               f"d{wl.head_dim} {wl.dtype}, budget {wl.budget}, chunk {wl.chunk_tokens}, probe {wl.probe_tokens}, "
+                               f"T {work['T']}", "streams_per_gpu": B, "parallelism": f"replicas x{world} (independent streams, no collective)",
+                   "l2": "working set per step (K+V read 370 MB + 360 MB written) exceeds the 126 MB L2; inputs cycle through "
+                         f"{POOL} chunk/probe sets", "score_path": score_path},
+        "e2e": {"value": job_value(wl, world, B, ms_e2e), "unit": UNIT, "ms_per_step": ms_e2e,
+                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e},
+        "gpu_launches": launches,
+        "kernel_ms": kern,
+        "roofline": roof,
+        "roofline_step": step_roof,
+        "clocks": clocks,
+    }
+    hb.hermes_destroy(h)
+    return out
+
+
+# ------------------------------------------------------------------------------- oracle timing (CPU)
+def oracle_sample(wl, steps: int, n_layers_sample: int, warmup: int = 0):
+    """Times oracle_step, as it stands, on a bounded sample: the full-geometry cache (budget, chunk, probe,
+    heads, head_dim) with `n_layers_sample` layers, in steady state.  Returns (seconds per step, threads)."""
+    from oracle import hermes_oracle as ho
+    swl = wl.scaled(n_layers=n_layers_sample, n_streams=1)
+    cfg = ho.OracleConfig(n_layers=swl.n_layers, n_q_heads=swl.n_q_heads, n_kv_heads=swl.n_kv_heads,
+                          head_dim=swl.head_dim, budget=swl.budget, forget_rate=swl.k_forget, dtype=swl.dtype,
+                          rope_mode=swl.rope_mode, rope_theta=swl.rope_theta, mrope_section=swl.mrope_section,
+                          mrope_compact_axes=swl.mrope_compact_axes, pos_offset=swl.pos_offset, capacity=swl.cap)
+    st = ho.OracleStream(cfg)
+    K, V, _ = chunk_kv(swl, 0, 0, 0, swl.budget)
+    ho.oracle_step(st, K, V, None)
+    times = []
+    for u in range(warmup + steps):
+        K, V, _ = chunk_kv(swl, 0, 1 + u, swl.budget + u * swl.chunk_tokens, swl.chunk_tokens)
+        Q = probe_q(swl, 0, 1 + u)
+        t0 = time.perf_counter()
+        ho.oracle_step(st, K, V, Q)
+        times.append(time.perf_counter() - t0)
+    times = times[warmup:]
+    try:
+        from threadpoolctl import threadpool_info
+        threads = max([p.get("num_threads", 1) for p in threadpool_info()] or [1])
+    except Exception:
+        threads = len(os.sched_getaffinity(0))
+    return sum(times) / len(times), threads, swl
+
+
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return None
+    wl = CONFIGS[args.workload]
+    Ls = 4                                                   # 1 shallow + 2 middle + 1 deep (10/60/30 % rule at L = 4)
+    sec, threads, swl = oracle_sample(wl, args.steps, Ls, warmup=min(args.warmup, 2))
+    T = wl.budget + wl.chunk_tokens
+    val = Ls * T / sec
+    sample = (f"oracle_step on {Ls} of {wl.n_layers} layers (1 shallow, 2 middle, 1 deep) of the full-geometry cache "
+              f"(T {T}, budget {wl.budget}, probe {wl.probe_tokens}), steady state, per step")
+    return {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": min(args.warmup, 2), "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[1] {wl.name} (bounded sample: {Ls} layers)"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=256)
+    ap.add_argument("--warmup", type=int, default=8)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="llava_ov_7b", choices=sorted(CONFIGS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        out = run_reference(args)
+    else:
+        out = run_ours(args)
+        rank, _, world = dist_env()
+        if out is not None and world == 1 and not args.no_cpu_baseline:
+            wl = CONFIGS[args.workload]
+            sec, threads, swl = oracle_sample(wl, 2, wl.n_layers)       # two full-size oracle updates
+            T = wl.budget + wl.chunk_tokens
+            out["cpu_baseline"] = {"value": wl.n_layers * T / sec, "unit": UNIT, "cores": threads, "kind": "oracle",
+                                   "ms_per_step": sec * 1e3,
+                                   "sample": f"2 full-size oracle_step updates of one stream ({wl.n_layers} layers, T {T}) in steady state"}
+    if out is not None:
+        print(json.dumps(out))
+
+
+if __name__ == "__main__":
+    main()
