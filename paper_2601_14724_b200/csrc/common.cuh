@@ -23,10 +23,11 @@ struct Geom {
   int compact_axes;
   int grid_h, grid_w;
   int table_rows;   // rotary table covers delta in [-(table_rows-1), 0]
+  int n_vh_max;     // column-sum slots per (stream, layer): Hkv * max row super-chunks per KV head
   void* kc;         // K cache   [B*L*2][cap][row_elems]
   void* vc;         // V cache   same
   int32_t* posc;    // positions [B*L*2][n_axes][cap]
-  float* colsum;    // [B*L][Hkv][cap]   per-KV-head column sums of the softmax (a1)
+  float* colsum;    // [B*L][n_vh_max][cap] per-(KV head, row super-chunk) column sums of the softmax (a1)
   float* rowstat;   // [B*L][Hq*p_max][2] (m2, 1/Z) per probe row, log2 domain
   float* partial;   // [B*L][Hq*p_max][n_part_max][2] partial (m2, z)
   float* scores;    // [B*L][cap]  smoothed scores S~ of the last eviction (a3)

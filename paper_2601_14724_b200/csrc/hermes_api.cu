@@ -88,7 +88,7 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   g.n_shallow = y.n_shallow; g.p_max = c->max_probe_tokens; g.pos_offset = c->pos_offset;
   g.sec_t = c->mrope_section[0]; g.sec_h = c->mrope_section[1];
   g.compact_axes = c->mrope_compact_axes; g.grid_h = c->mrope_grid_h; g.grid_w = c->mrope_grid_w;
-  g.table_rows = y.table_rows;
+  g.table_rows = y.table_rows; g.n_vh_max = y.n_vh_max;
   g.kc = h->ws + y.kc; g.vc = h->ws + y.vc; g.posc = reinterpret_cast<int32_t*>(h->ws + y.posc);
   g.colsum = reinterpret_cast<float*>(h->ws + y.colsum);
   g.rowstat = reinterpret_cast<float*>(h->ws + y.rowstat);
@@ -285,13 +285,14 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
         if (c.dtype == HERMES_BF16) launch_simt<__nv_bfloat16>(h, Q_probe, Tn, n_probe, scale_log2, s);
         else launch_simt<float>(h, Q_probe, Tn, n_probe, scale_log2, s);
         h->last_score_path = HERMES_SCORE_SIMT;
+        h->n_vh = g.Hkv;
       }
     }
     {
       Prof p(h, HERMES_K_SELECT, s);
       const double k = c.forget_rate;
       const float r_norm_sum = float((1.0 - std::exp(-k)) / (1.0 - std::exp(-k * Tn)));
-      k_select<<<BL, kSelThreads, size_t(Tn) * 4, s>>>(g, h->cur, Tn, n_probe, c.forget_rate, c.norm_mode == HERMES_NORM_SUM, r_norm_sum);
+      k_select<<<BL, kSelThreads, size_t(Tn) * 4, s>>>(g, h->cur, Tn, n_probe, c.forget_rate, c.norm_mode == HERMES_NORM_SUM, r_norm_sum, h->n_vh);
     }
     {
       Prof p(h, HERMES_K_GATHER, s);

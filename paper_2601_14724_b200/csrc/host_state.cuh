@@ -17,7 +17,7 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 struct Layout {           // byte offsets into the workspace
   size_t kc, vc, posc, colsum, rowstat, partial, scores, kept, rope_tab, rope_freq, omega, lambda,
       status, stage_k, stage_v, stage_q, tmaps, total;
-  int cap, n_axes, n_part_max, table_rows, n_shallow, n_middle, n_deep;
+  int cap, n_axes, n_part_max, table_rows, n_shallow, n_middle, n_deep, n_vh_max;
   size_t esize, row_bytes;
 };
 
@@ -68,6 +68,7 @@ inline Layout make_layout(const hermes_config& c) {
   y.esize = c.dtype == HERMES_BF16 ? 2 : 4;
   y.row_bytes = size_t(c.n_kv_heads) * c.head_dim * y.esize;
   y.n_part_max = (y.cap + 127) / 128;
+  y.n_vh_max = c.n_kv_heads * std::max(1, (c.n_q_heads / c.n_kv_heads * c.max_probe_tokens + 511) / 512);
   int ns = c.n_shallow, nd = c.n_deep;
   stage_split(c.n_layers, ns, nd);
   y.n_shallow = ns; y.n_deep = nd; y.n_middle = c.n_layers - ns - nd;
@@ -84,7 +85,7 @@ inline Layout make_layout(const hermes_config& c) {
   y.kc = take(BL * 2 * y.cap * y.row_bytes);
   y.vc = take(BL * 2 * y.cap * y.row_bytes);
   y.posc = take(BL * 2 * y.n_axes * y.cap * 4);
-  y.colsum = take(BL * c.n_kv_heads * y.cap * 4);
+  y.colsum = take(BL * y.n_vh_max * y.cap * 4);
   y.rowstat = take(BL * rows * 2 * 4);
   y.partial = take(BL * rows * y.n_part_max * 2 * 4);
   y.scores = take(BL * y.cap * 4);
@@ -122,6 +123,7 @@ struct hermes {
   int last_T = 0;
   int last_score_path = 0;
   int last_launches = 0;
+  int n_vh = 0;             // column-sum slots written by the last scoring pass
   bool profiling = false;
   bool tc_ok = false;       // tcgen05 scoring path usable for this config + device
   hk::KernelTimer timer;

@@ -106,7 +106,7 @@ k_score_simt(Geom g, const T* __restrict__ q_probe, int cur, int Tn, int P, floa
       }
     }
   }
-  if (kColsum && valid) g.colsum[(size_t(bl) * g.Hkv + kvh) * g.cap + tok] = acc_w;
+  if (kColsum && valid) g.colsum[(size_t(bl) * g.n_vh_max + kvh) * g.cap + tok] = acc_w;
 }
 
 // Per probe row: merge n_part partial (m2, z) into (m2, 1/Z).  One warp per row.

@@ -74,15 +74,15 @@ __device__ inline int block_reduce_min_i(int v, int* scratch) {
 }
 
 // W of one layer at token i: per-KV-head column sums added in fixed head order, / (Hq * P).
-__device__ inline float mean_w(const Geom& g, int bl, int i, float inv_rows) {
-  const float* c = g.colsum + size_t(bl) * g.Hkv * g.cap + i;
+__device__ inline float mean_w(const Geom& g, int bl, int i, float inv_rows, int n_vh) {
+  const float* c = g.colsum + size_t(bl) * g.n_vh_max * g.cap + i;
   float w = 0.f;
-  for (int h = 0; h < g.Hkv; ++h) w += c[size_t(h) * g.cap];
+  for (int h = 0; h < n_vh; ++h) w += c[size_t(h) * g.cap];
   return w * inv_rows;
 }
 
 __global__ void __launch_bounds__(kSelThreads)
-k_select(Geom g, int cur, int Tn, int P, float k_forget, int norm_sum, float r_norm_sum) {
+k_select(Geom g, int cur, int Tn, int P, float k_forget, int norm_sum, float r_norm_sum, int n_vh) {
   extern __shared__ float s_sc[];                    // [Tn] smoothed scores
   __shared__ int hist[256];
   __shared__ int warp_tot[33];
@@ -103,8 +103,8 @@ k_select(Geom g, int cur, int Tn, int P, float k_forget, int norm_sum, float r_n
   // ---- a2: per-layer normalisation factor alpha (max or sum of W) ------------------------------
   float n0 = 0.f, n1 = 0.f;
   for (int i = tid; i < Tn; i += kSelThreads) {
-    if (scored0) { const float w = mean_w(g, bl, i, inv_rows); n0 = norm_sum ? n0 + w : fmaxf(n0, w); }
-    if (scored1) { const float w = mean_w(g, bl + 1, i, inv_rows); n1 = norm_sum ? n1 + w : fmaxf(n1, w); }
+    if (scored0) { const float w = mean_w(g, bl, i, inv_rows, n_vh); n0 = norm_sum ? n0 + w : fmaxf(n0, w); }
+    if (scored1) { const float w = mean_w(g, bl + 1, i, inv_rows, n_vh); n1 = norm_sum ? n1 + w : fmaxf(n1, w); }
   }
   n0 = norm_sum ? block_reduce_sum(n0, red_f) : block_reduce_max(n0, red_f);
   n1 = norm_sum ? block_reduce_sum(n1, red_f) : block_reduce_max(n1, red_f);
@@ -117,10 +117,10 @@ k_select(Geom g, int cur, int Tn, int P, float k_forget, int norm_sum, float r_n
   float* scores_out = g.scores + size_t(bl) * g.cap;
   for (int i = tid; i < Tn; i += kSelThreads) {
     const float R = expf(-k_forget * float(Tn - 1 - i)) * r_norm;           // Eq. 1
-    const float A0 = scored0 ? mean_w(g, bl, i, inv_rows) * a0 : 0.f;       // Eq. 2
+    const float A0 = scored0 ? mean_w(g, bl, i, inv_rows, n_vh) * a0 : 0.f;       // Eq. 2
     float s = (1.0f - om0) * A0 + om0 * R;                                   // Eq. 4
     if (has_next) {
-      const float A1 = scored1 ? mean_w(g, bl + 1, i, inv_rows) * a1 : 0.f;
+      const float A1 = scored1 ? mean_w(g, bl + 1, i, inv_rows, n_vh) * a1 : 0.f;
       const float s1 = (1.0f - om1) * A1 + om1 * R;
       s = (1.0f - lam) * s + lam * s1;                                       // Eq. 5
     }
