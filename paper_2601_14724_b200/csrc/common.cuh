@@ -32,6 +32,7 @@ struct Geom {
   float* partial;   // [B*L][Hq*p_max][n_part_max][2] partial (m2, z)
   float* scores;    // [B*L][cap]  smoothed scores S~ of the last eviction (a3)
   int32_t* kept;    // [B*L][budget] ascending kept indices I_l (a4)
+  int32_t* delta;   // [B*L][n_axes][budget] p_new - p_old of every kept token (a6 -> a7)
   float2* rope_tab; // [table_rows][d/2] (cos, sin)(-r * theta_j) for r = row index
   double* rope_freq;// [d/2] theta_j in fp64 (slow path for deltas outside the table)
   float* omega;     // [L] weight of the recency term (Eq. 3-4); 1 shallow, 0 deep
@@ -88,6 +89,13 @@ __device__ inline uint4 ldg_stream(const void* p) {  // streaming 128-bit load, 
 __device__ inline void stg_stream(void* p, const uint4& v) {
   asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};"
                :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+// 2^x on the MUFU pipe (ex2.approx.ftz: rel. error <= 2^-22, ex2(-inf) = +0); exp2f() costs 4 instructions
+__device__ __forceinline__ float fast_exp2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
 }
 
 __device__ inline float warp_max(float v) {

@@ -75,11 +75,13 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   if (size_t(y.cap) * 4 + 24 * 1024 > prop.sharedMemPerBlockOptin)
     return fail(nullptr, HERMES_EINVAL, "max_tokens %d too large for the select kernel's shared memory", y.cap);
   CUDA_TRY(nullptr, cudaSetDevice(c->device));
+  const int n_sm = prop.multiProcessorCount;
 
   hermes_t* h = new (std::nothrow) hermes;
   if (!h) return fail(nullptr, HERMES_ENOMEM, "out of host memory");
   h->cfg = *c; h->lay = y; h->ws = static_cast<char*>(workspace);
   h->next_pos = c->pos_offset;
+  h->n_sm = n_sm;
 
   Geom& g = h->geom;
   g.B = c->n_streams; g.L = c->n_layers; g.Hq = c->n_q_heads; g.Hkv = c->n_kv_heads;
@@ -95,6 +97,7 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   g.partial = reinterpret_cast<float*>(h->ws + y.partial);
   g.scores = reinterpret_cast<float*>(h->ws + y.scores);
   g.kept = reinterpret_cast<int32_t*>(h->ws + y.kept);
+  g.delta = reinterpret_cast<int32_t*>(h->ws + y.delta);
   g.rope_tab = reinterpret_cast<float2*>(h->ws + y.rope_tab);
   g.rope_freq = reinterpret_cast<double*>(h->ws + y.rope_freq);
   g.omega = reinterpret_cast<float*>(h->ws + y.omega);
@@ -299,9 +302,17 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
       const int V = c.dtype == HERMES_BF16 ? 8 : 4;
       const int upr = g.Hkv * (g.d / 2 / V);
       const int total = g.budget * upr;
-      const int gx = std::max(1, (total + 2 * kGatherThreads - 1) / (2 * kGatherThreads));
-      if (c.dtype == HERMES_BF16) k_gather<__nv_bfloat16><<<dim3(gx, BL), kGatherThreads, 0, s>>>(g, h->cur);
-      else k_gather<float><<<dim3(gx, BL), kGatherThreads, 0, s>>>(g, h->cur);
+      // ~4 resident blocks per SM over all slabs; every thread walks total / (gx * 256) units
+      const int want = std::max(1, (h->n_sm * 4 * 2 + BL - 1) / BL);
+      const int gx = std::max(1, std::min(want, (total + kGatherThreads - 1) / kGatherThreads));
+      const dim3 grid(gx, BL);
+      if (c.dtype == HERMES_BF16) {
+        if (g.n_axes == 1) k_gather<__nv_bfloat16, 1><<<grid, kGatherThreads, 0, s>>>(g, h->cur);
+        else k_gather<__nv_bfloat16, 3><<<grid, kGatherThreads, 0, s>>>(g, h->cur);
+      } else {
+        if (g.n_axes == 1) k_gather<float, 1><<<grid, kGatherThreads, 0, s>>>(g, h->cur);
+        else k_gather<float, 3><<<grid, kGatherThreads, 0, s>>>(g, h->cur);
+      }
     }
   }
   cudaError_t e = cudaGetLastError();

@@ -15,7 +15,7 @@ namespace hk {
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {           // byte offsets into the workspace
-  size_t kc, vc, posc, colsum, rowstat, partial, scores, kept, rope_tab, rope_freq, omega, lambda,
+  size_t kc, vc, posc, colsum, rowstat, partial, scores, kept, delta, rope_tab, rope_freq, omega, lambda,
       status, stage_k, stage_v, stage_q, tmaps, total;
   int cap, n_axes, n_part_max, table_rows, n_shallow, n_middle, n_deep, n_vh_max;
   size_t esize, row_bytes;
@@ -90,6 +90,7 @@ inline Layout make_layout(const hermes_config& c) {
   y.partial = take(BL * rows * y.n_part_max * 2 * 4);
   y.scores = take(BL * y.cap * 4);
   y.kept = take(BL * c.budget * 4);
+  y.delta = take(BL * y.n_axes * c.budget * 4);
   y.rope_tab = take(size_t(y.table_rows) * (c.head_dim / 2) * 8);
   y.rope_freq = take(size_t(c.head_dim / 2) * 8);
   y.omega = take(size_t(c.n_layers) * 4);
@@ -123,6 +124,7 @@ struct hermes {
   int last_T = 0;
   int last_score_path = 0;
   int last_launches = 0;
+  int n_sm = 148;
   int n_vh = 0;             // column-sum slots written by the last scoring pass
   bool profiling = false;
   bool tc_ok = false;       // tcgen05 scoring path usable for this config + device

@@ -200,14 +200,21 @@ k_tc_stats(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ C
         if (lane == 0) ptx::mbar_arrive(&t_empty[as]);                  // values are in registers: free the stage
         if (active) {
           const int n_valid = min(TN, a.Tn - t * TN);                   // ragged last tile of the group
-          float mx = -INFINITY;
+          if (n_valid < TN) {
 #pragma unroll
-          for (int j = 0; j < TN; ++j) { if (j >= n_valid) v[j] = -INFINITY; mx = fmaxf(mx, v[j]); }
-          const float m_new = fmaxf(m_run, mx * a.scale_log2);
-          float acc = 0.f;
+            for (int j = 0; j < TN; ++j) if (j >= n_valid) v[j] = -INFINITY;
+          }
+          float mx0 = v[0], mx1 = v[1];
 #pragma unroll
-          for (int j = 0; j < TN; ++j) acc += exp2f(fmaf(v[j], a.scale_log2, -m_new));
-          z = z * exp2f(m_run - m_new) + acc;
+          for (int j = 2; j < TN; j += 2) { mx0 = fmaxf(mx0, v[j]); mx1 = fmaxf(mx1, v[j + 1]); }
+          const float m_new = fmaxf(m_run, fmaxf(mx0, mx1) * a.scale_log2);
+          float acc0 = 0.f, acc1 = 0.f;
+#pragma unroll
+          for (int j = 0; j < TN; j += 2) {
+            acc0 += fast_exp2(fmaf(v[j], a.scale_log2, -m_new));
+            acc1 += fast_exp2(fmaf(v[j + 1], a.scale_log2, -m_new));
+          }
+          z = z * fast_exp2(m_run - m_new) + (acc0 + acc1);
           m_run = m_new;
         }
         if (++as == 2) { as = 0; aph ^= 1; }
@@ -335,31 +342,38 @@ k_tc_colsum(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ 
             float m = -INFINITY;
             for (int j = 0; j < a.spg; ++j) m = fmaxf(m, p2[j].x);
             float z = 0.f;
-            for (int j = 0; j < a.spg; ++j) z += p2[j].y * exp2f(p2[j].x - m);
+            for (int j = 0; j < a.spg; ++j) z += p2[j].y * fast_exp2(p2[j].x - m);
             c = m + log2f(z);
           }
           s.c[i] = c;
         }
         ptx::named_bar_sync(1, 256);
       }
-      float acc = 0.f;
+      float acc = 0.f, acc2 = 0.f;
       for (int c0 = 0; c0 < rs32; c0 += 256) {
         const int nc = min(256, rs32 - c0);
         ptx::mbar_wait(&t_full[as], aph);
         ptx::tc_fence_after();
-        for (int b0 = half * 32; b0 < nc; b0 += 64) {                    // this warp's 32-column blocks
-          float v[32];
-          ptx::tmem_ld32(tmem_base + (uint32_t(lg * 32) << 16) + as * 256 + b0, v);
+        // this warp's 32-column blocks b0, b0+64, ...: the next block's TMEM load is in flight while
+        // the current one goes through the MUFU pipe
+        const uint32_t tbase = tmem_base + (uint32_t(lg * 32) << 16) + as * 256;
+        float v[2][32];
+        int b0 = half * 32, cur_buf = 0;
+        if (b0 < nc) ptx::tmem_ld32(tbase + b0, v[0]);
+        for (; b0 < nc; b0 += 64) {
           ptx::tmem_ld_wait();
+          if (b0 + 64 < nc) ptx::tmem_ld32(tbase + b0 + 64, v[cur_buf ^ 1]);
           const float4* c4 = reinterpret_cast<const float4*>(s.c + c0 + b0);
+          const float* vv = v[cur_buf];
 #pragma unroll
           for (int j = 0; j < 8; ++j) {
             const float4 c = c4[j];
-            acc += exp2f(fmaf(v[4 * j], a.scale_log2, -c.x));
-            acc += exp2f(fmaf(v[4 * j + 1], a.scale_log2, -c.y));
-            acc += exp2f(fmaf(v[4 * j + 2], a.scale_log2, -c.z));
-            acc += exp2f(fmaf(v[4 * j + 3], a.scale_log2, -c.w));
+            acc += fast_exp2(fmaf(vv[4 * j], a.scale_log2, -c.x));
+            acc2 += fast_exp2(fmaf(vv[4 * j + 1], a.scale_log2, -c.y));
+            acc += fast_exp2(fmaf(vv[4 * j + 2], a.scale_log2, -c.z));
+            acc2 += fast_exp2(fmaf(vv[4 * j + 3], a.scale_log2, -c.w));
           }
+          cur_buf ^= 1;
         }
         ptx::tc_fence_before();
         __syncwarp();
@@ -367,6 +381,7 @@ k_tc_colsum(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ 
         if (++as == 2) { as = 0; aph ^= 1; }
       }
       // merge the two column halves and store W's per-(KV head, super-chunk) column sum of this token
+      acc += acc2;
       if (half == 1) acc_x[tok_in_tile] = acc;
       ptx::named_bar_sync(2, 256);
       if (half == 0) {

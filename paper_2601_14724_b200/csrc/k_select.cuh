@@ -208,14 +208,19 @@ k_select(Geom g, int cur, int Tn, int P, float k_forget, int norm_sum, float r_n
   const int32_t* pos_old = g.posc + (size_t(bl) * 2 + cur) * g.n_axes * g.cap;
   int32_t* pos_new = g.posc + (size_t(bl) * 2 + (cur ^ 1)) * g.n_axes * g.cap;
   if (g.n_axes == 1) {                                  // Eq. 8: positions increase with the index -> rank = slot
-    for (int s = tid; s < g.budget; s += kSelThreads) pos_new[s] = g.pos_offset + s;
+    int32_t* dl = g.delta + size_t(bl) * g.budget;
+    for (int s = tid; s < g.budget; s += kSelThreads) {
+      pos_new[s] = g.pos_offset + s;
+      dl[s] = g.pos_offset + s - pos_old[kept[s]];
+    }
     return;
   }
   for (int a = 0; a < 3; ++a) {
     const int32_t* po = pos_old + size_t(a) * g.cap;
     int32_t* pn = pos_new + size_t(a) * g.cap;
+    int32_t* dl = g.delta + (size_t(bl) * 3 + a) * g.budget;
     if (!((g.compact_axes >> a) & 1)) {                 // axis kept as is (DESIGN c13)
-      for (int s = tid; s < g.budget; s += kSelThreads) pn[s] = po[kept[s]];
+      for (int s = tid; s < g.budget; s += kSelThreads) { pn[s] = po[kept[s]]; dl[s] = 0; }
       continue;
     }
     int vmin = INT_MAX, vmax_neg = INT_MAX;
@@ -227,7 +232,7 @@ k_select(Geom g, int cur, int Tn, int P, float k_forget, int norm_sum, float r_n
     const int vmax = -block_reduce_min_i(vmax_neg, red_i);
     if (vmax - vmin >= kBitmapWords * 32) {             // cannot rank: report, leave the axis untouched
       if (tid == 0) atomicOr(g.status, 1);
-      for (int s = tid; s < g.budget; s += kSelThreads) pn[s] = po[kept[s]];
+      for (int s = tid; s < g.budget; s += kSelThreads) { pn[s] = po[kept[s]]; dl[s] = 0; }
       continue;
     }
     for (int w = tid; w < kBitmapWords; w += kSelThreads) bitmap[w] = 0u;
@@ -245,7 +250,9 @@ k_select(Geom g, int cur, int Tn, int P, float k_forget, int norm_sum, float r_n
     __syncthreads();
     for (int s = tid; s < g.budget; s += kSelThreads) {  // Eq. 11: offset + rank among distinct coordinates
       const int v = po[kept[s]] - vmin;
-      pn[s] = g.pos_offset + word_prefix[v >> 5] + __popc(bitmap[v >> 5] & ((1u << (v & 31)) - 1u));
+      const int p_new = g.pos_offset + word_prefix[v >> 5] + __popc(bitmap[v >> 5] & ((1u << (v & 31)) - 1u));
+      pn[s] = p_new;
+      dl[s] = p_new - (v + vmin);
     }
     __syncthreads();
   }
