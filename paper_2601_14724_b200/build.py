@@ -30,7 +30,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not needs_build():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc, *NVCC_FLAGS, "-o", LIB, os.path.join(CSRC, "hermes_api.cu")]
+    cmd = [nvcc, *NVCC_FLAGS, *os.environ.get("HERMES_NVCC_EXTRA", "").split(), "-o", LIB, os.path.join(CSRC, "hermes_api.cu")]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     r = subprocess.run(cmd, capture_output=True, text=True)

@@ -28,6 +28,8 @@ struct Geom {
   void* vc;         // V cache   same
   int32_t* posc;    // positions [B*L*2][n_axes][cap]
   float* colsum;    // [B*L][n_vh_max][cap] per-(KV head, row super-chunk) column sums of the softmax (a1)
+  float* wsum;      // [B*L][cap] W_i: column sums added over KV heads / (Hq*P)  (Eq. 2)
+  uint32_t* wmax;   // [B*L] max_i W_i as float bits (W >= 0), zeroed by k_append
   float* rowstat;   // [B*L][Hq*p_max][2] (m2, 1/Z) per probe row, log2 domain
   float* partial;   // [B*L][Hq*p_max][n_part_max][2] partial (m2, z)
   float* scores;    // [B*L][cap]  smoothed scores S~ of the last eviction (a3)

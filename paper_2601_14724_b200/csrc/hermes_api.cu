@@ -94,6 +94,8 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   g.kc = h->ws + y.kc; g.vc = h->ws + y.vc; g.posc = reinterpret_cast<int32_t*>(h->ws + y.posc);
   g.colsum = reinterpret_cast<float*>(h->ws + y.colsum);
   g.rowstat = reinterpret_cast<float*>(h->ws + y.rowstat);
+  g.wsum = reinterpret_cast<float*>(h->ws + y.wsum);
+  g.wmax = reinterpret_cast<uint32_t*>(h->ws + y.wmax);
   g.partial = reinterpret_cast<float*>(h->ws + y.partial);
   g.scores = reinterpret_cast<float*>(h->ws + y.scores);
   g.kept = reinterpret_cast<int32_t*>(h->ws + y.kept);
@@ -293,9 +295,12 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
     }
     {
       Prof p(h, HERMES_K_SELECT, s);
+      if (g.L > g.n_shallow) ++h->last_launches;
       const double k = c.forget_rate;
       const float r_norm_sum = float((1.0 - std::exp(-k)) / (1.0 - std::exp(-k * Tn)));
-      k_select<<<BL, kSelThreads, size_t(Tn) * 4, s>>>(g, h->cur, Tn, n_probe, c.forget_rate, c.norm_mode == HERMES_NORM_SUM, r_norm_sum, h->n_vh);
+      if (g.L > g.n_shallow)
+        k_wsum<<<dim3((Tn + 255) / 256, g.B * (g.L - g.n_shallow)), 256, 0, s>>>(g, Tn, n_probe, h->n_vh);
+      k_select<<<BL, kSelThreads, size_t(Tn) * 4, s>>>(g, h->cur, Tn, c.forget_rate, c.norm_mode == HERMES_NORM_SUM, r_norm_sum);
     }
     {
       Prof p(h, HERMES_K_GATHER, s);

@@ -15,7 +15,7 @@ namespace hk {
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {           // byte offsets into the workspace
-  size_t kc, vc, posc, colsum, rowstat, partial, scores, kept, delta, rope_tab, rope_freq, omega, lambda,
+  size_t kc, vc, posc, colsum, wsum, wmax, rowstat, partial, scores, kept, delta, rope_tab, rope_freq, omega, lambda,
       status, stage_k, stage_v, stage_q, tmaps, total;
   int cap, n_axes, n_part_max, table_rows, n_shallow, n_middle, n_deep, n_vh_max;
   size_t esize, row_bytes;
@@ -86,6 +86,8 @@ inline Layout make_layout(const hermes_config& c) {
   y.vc = take(BL * 2 * y.cap * y.row_bytes);
   y.posc = take(BL * 2 * y.n_axes * y.cap * 4);
   y.colsum = take(BL * y.n_vh_max * y.cap * 4);
+  y.wsum = take(BL * y.cap * 4);
+  y.wmax = take(BL * 4);
   y.rowstat = take(BL * rows * 2 * 4);
   y.partial = take(BL * rows * y.n_part_max * 2 * 4);
   y.scores = take(BL * y.cap * 4);

@@ -11,6 +11,7 @@ __global__ void __launch_bounds__(256)
 k_append(Geom g, const uint4* __restrict__ k_new, const uint4* __restrict__ v_new,
          int cur, int len, int n_new, int row_vecs, int pos_start) {
   const int bl = blockIdx.y;                        // b * L + l
+  if (blockIdx.x == 0 && threadIdx.x == 0) g.wmax[bl] = 0u;   // reset the per-layer max of W for this step
   const size_t slab = size_t(bl) * 2 + cur;
   const size_t n_vec = size_t(n_new) * row_vecs;
   const uint4* ks = k_new + size_t(bl) * n_vec;

@@ -20,7 +20,7 @@ constexpr int kTcRowsMax = 512;                 // probe rows resident per group
 constexpr int kTcQHalfBytes = kTcRowsMax * 128; // one 64-column half of the Q tile
 constexpr int kTcKBytes = 64 * 1024;            // K ring: 4 x 16 KB (pass 1) or 2 x 32 KB (pass 2)
 constexpr int kTcSmemBytes = 2 * kTcQHalfBytes + kTcKBytes + kTcRowsMax * 4 + 512 + 1024;
-constexpr int kTcStatsThreads = 64 + 16 * 32;   // producer, MMA, 16 epilogue warps
+constexpr int kTcStatsThreads = 64 + 8 * 32;    // producer, MMA, 8 epilogue warps
 constexpr int kTcColsumThreads = 64 + 8 * 32;   // producer, MMA, 8 epilogue warps
 constexpr int kTcSegTiles = 8;                  // pass 1: 64-token tiles per segment (one partial per segment,
                                                 // so the merge order never depends on the CTA schedule)
@@ -103,7 +103,7 @@ k_tc_stats(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ C
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tmap(&tmap_q); ptx::prefetch_tmap(&tmap_k);
     for (int i = 0; i < NS; ++i) { ptx::mbar_init(&k_full[i], 1); ptx::mbar_init(&k_empty[i], 1); }
-    for (int i = 0; i < 2; ++i) { ptx::mbar_init(&t_full[i], 1); ptx::mbar_init(&t_empty[i], 16); }
+    for (int i = 0; i < 2; ++i) { ptx::mbar_init(&t_full[i], 1); ptx::mbar_init(&t_empty[i], 8); }
     ptx::mbar_init(q_full, 1); ptx::mbar_init(q_empty, 1);
     ptx::fence_barrier_init();
   }
@@ -174,54 +174,87 @@ k_tc_stats(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ C
       }
     }
   } else {
-    // ---------------- epilogue: one probe row per thread ----------------
-    const int e = warp - 2, rb = e >> 2, lg = warp & 3;
-    const int row = rb * 128 + lg * 32 + lane;
-    int as = 0, aph = 0, prev = -1;
-    TcGroup gr{};
-    for (long long u = s0; u < s1; ++u) {
-      const int gi = int(u / a.spg), sg = int(u % a.spg);
-      if (gi != prev) { gr = tc_group(a, gi); prev = gi; }
-      const bool active = rb * 128 + lg * 32 < gr.rs_valid;            // warp-uniform
-      float m_run = -INFINITY, z = 0.f;
-      const int t_end = min(a.tpg, (sg + 1) * kTcSegTiles);
-      for (int t = sg * kTcSegTiles; t < t_end; ++t) {
-        ptx::mbar_wait(&t_full[as], aph);
-        ptx::tc_fence_after();
-        float v[TN];
-        if (active) {
-          const uint32_t taddr = tmem_base + (uint32_t(lg * 32) << 16) + as * 256 + rb * TN;
-          ptx::tmem_ld32(taddr, v);
-          ptx::tmem_ld32(taddr + 32, v + 32);
-          ptx::tmem_ld_wait();
-        }
+    // ---------------- epilogue: two probe rows per thread (row blocks rb0, rb0+1), software-pipelined:
+    // the TMEM load of one row block is always in flight while the other goes through the MUFU pipe ----
+    const int e = warp - 2, rb0 = (e >> 2) * 2, lg = warp & 3;
+    int as = 0, aph = 0;
+    float m_run[2] = {-INFINITY, -INFINITY}, z[2] = {0.f, 0.f};
+    float vA[TN], vB[TN];
+    // running (max, sum exp2) of one row over one 64-token tile
+    auto fold = [&](float (&v)[TN], int t, float& m_r, float& z_r) {
+      const int n_valid = min(TN, a.Tn - t * TN);                       // ragged last tile of the group
+      if (n_valid < TN) {
+#pragma unroll
+        for (int j = 0; j < TN; ++j) if (j >= n_valid) v[j] = -INFINITY;
+      }
+      float mx[4] = {v[0], v[1], v[2], v[3]};
+#pragma unroll
+      for (int j = 4; j < TN; j += 4) {
+        mx[0] = fmaxf(mx[0], v[j]); mx[1] = fmaxf(mx[1], v[j + 1]);
+        mx[2] = fmaxf(mx[2], v[j + 2]); mx[3] = fmaxf(mx[3], v[j + 3]);
+      }
+      const float m_new = fmaxf(m_r, fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])) * a.scale_log2);
+#pragma unroll
+      for (int j = 0; j < TN; ++j) v[j] = fmaf(v[j], a.scale_log2, -m_new);
+#pragma unroll
+      for (int j = 0; j < TN; ++j) v[j] = fast_exp2(v[j]);
+      float sm[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+      for (int j = 0; j < TN; j += 4) { sm[0] += v[j]; sm[1] += v[j + 1]; sm[2] += v[j + 2]; sm[3] += v[j + 3]; }
+      z_r = z_r * fast_exp2(m_r - m_new) + ((sm[0] + sm[1]) + (sm[2] + sm[3]));
+      m_r = m_new;
+    };
+    long long u = s0;
+    if (u < s1) {
+      int gi = int(u / a.spg), sg = int(u % a.spg);
+      TcGroup gr = tc_group(a, gi);
+      int t = sg * kTcSegTiles, t_end = min(a.tpg, t + kTcSegTiles);
+      bool act0 = rb0 * 128 + lg * 32 < gr.rs_valid, act1 = (rb0 + 1) * 128 + lg * 32 < gr.rs_valid;
+      const uint32_t lane_base = uint32_t(lg * 32) << 16;
+      ptx::mbar_wait(&t_full[as], aph);
+      ptx::tc_fence_after();
+      if (act0) { ptx::tmem_ld32(tmem_base + lane_base + as * 256 + rb0 * TN, vA); ptx::tmem_ld32(tmem_base + lane_base + as * 256 + rb0 * TN + 32, vA + 32); }
+      while (true) {
+        ptx::tmem_ld_wait();                                             // row block rb0 of tile t is in registers
+        if (act1) { ptx::tmem_ld32(tmem_base + lane_base + as * 256 + (rb0 + 1) * TN, vB); ptx::tmem_ld32(tmem_base + lane_base + as * 256 + (rb0 + 1) * TN + 32, vB + 32); }
+        if (act0) fold(vA, t, m_run[0], z[0]);
+        ptx::tmem_ld_wait();                                             // row block rb0+1 too: free the TMEM stage
         ptx::tc_fence_before();
         __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(&t_empty[as]);                  // values are in registers: free the stage
-        if (active) {
-          const int n_valid = min(TN, a.Tn - t * TN);                   // ragged last tile of the group
-          if (n_valid < TN) {
-#pragma unroll
-            for (int j = 0; j < TN; ++j) if (j >= n_valid) v[j] = -INFINITY;
-          }
-          float mx0 = v[0], mx1 = v[1];
-#pragma unroll
-          for (int j = 2; j < TN; j += 2) { mx0 = fmaxf(mx0, v[j]); mx1 = fmaxf(mx1, v[j + 1]); }
-          const float m_new = fmaxf(m_run, fmaxf(mx0, mx1) * a.scale_log2);
-          float acc0 = 0.f, acc1 = 0.f;
-#pragma unroll
-          for (int j = 0; j < TN; j += 2) {
-            acc0 += fast_exp2(fmaf(v[j], a.scale_log2, -m_new));
-            acc1 += fast_exp2(fmaf(v[j + 1], a.scale_log2, -m_new));
-          }
-          z = z * fast_exp2(m_run - m_new) + (acc0 + acc1);
-          m_run = m_new;
-        }
+        if (lane == 0) ptx::mbar_arrive(&t_empty[as]);
         if (++as == 2) { as = 0; aph ^= 1; }
-      }
-      if (row < gr.rs_valid) {                                          // one partial per (row, segment)
-        float* out = a.g.partial + ((size_t(gr.bl) * a.g.Hq * a.g.p_max + gr.stat_row0 + row) * a.spg + sg) * 2;
-        out[0] = m_run; out[1] = z;
+        // advance to the next tile of this CTA's range and start its first load
+        const int t_cur = t, sg_cur = sg;
+        const TcGroup gr_cur = gr;
+        const bool seg_done = t + 1 >= t_end, act1_cur = act1;
+        bool more = true;
+        if (!seg_done) { ++t; }
+        else if (++u < s1) {
+          const int gi_n = int(u / a.spg);
+          sg = int(u % a.spg);
+          if (gi_n != gi) { gi = gi_n; gr = tc_group(a, gi); }
+          t = sg * kTcSegTiles; t_end = min(a.tpg, t + kTcSegTiles);
+        } else more = false;
+        const bool act0_cur = act0;
+        if (more) {
+          act0 = rb0 * 128 + lg * 32 < gr.rs_valid; act1 = (rb0 + 1) * 128 + lg * 32 < gr.rs_valid;
+          ptx::mbar_wait(&t_full[as], aph);
+          ptx::tc_fence_after();
+          if (act0) { ptx::tmem_ld32(tmem_base + lane_base + as * 256 + rb0 * TN, vA); ptx::tmem_ld32(tmem_base + lane_base + as * 256 + rb0 * TN + 32, vA + 32); }
+        }
+        if (act1_cur) fold(vB, t_cur, m_run[1], z[1]);
+        if (seg_done) {                                                  // one partial per (row, segment)
+#pragma unroll
+          for (int k = 0; k < 2; ++k) {
+            const int row = (rb0 + k) * 128 + lg * 32 + lane;
+            if ((k == 0 ? act0_cur : act1_cur) && row < gr_cur.rs_valid) {
+              float* out = a.g.partial + ((size_t(gr_cur.bl) * a.g.Hq * a.g.p_max + gr_cur.stat_row0 + row) * a.spg + sg_cur) * 2;
+              out[0] = m_run[k]; out[1] = z[k];
+            }
+            m_run[k] = -INFINITY; z[k] = 0.f;
+          }
+        }
+        if (!more) break;
       }
     }
   }
@@ -238,7 +271,7 @@ k_tc_colsum(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ 
   extern __shared__ uint8_t smem_raw[];
   const TcSmem s = tc_carve(smem_raw);
   constexpr int NS = 2, TN = 128, KSTAGE = 32768;
-  __shared__ float acc_x[128];          // partial sums of the upper column-half warps
+  __shared__ float acc_x[2][128];       // partial sums of the upper column-half warps (double-buffered)
   uint64_t* k_full = s.bars;            // [NS]
   uint64_t* k_empty = s.bars + NS;      // [NS]
   uint64_t* t_full = s.bars + 2 * NS;   // [2]
@@ -349,47 +382,59 @@ k_tc_colsum(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ 
         }
         ptx::named_bar_sync(1, 256);
       }
-      float acc = 0.f, acc2 = 0.f;
+      float acc[4] = {0.f, 0.f, 0.f, 0.f};
+      // 32 probe rows of this token: FFMA, MUFU and FADD phases kept apart so no warp waits on its own exp
+      auto fold = [&](float (&v)[32], int col) {
+        const float4* c4 = reinterpret_cast<const float4*>(s.c + col);
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const float4 c = c4[j];
+          v[4 * j] = fmaf(v[4 * j], a.scale_log2, -c.x);
+          v[4 * j + 1] = fmaf(v[4 * j + 1], a.scale_log2, -c.y);
+          v[4 * j + 2] = fmaf(v[4 * j + 2], a.scale_log2, -c.z);
+          v[4 * j + 3] = fmaf(v[4 * j + 3], a.scale_log2, -c.w);
+        }
+#pragma unroll
+        for (int j = 0; j < 32; ++j) v[j] = fast_exp2(v[j]);
+#pragma unroll
+        for (int j = 0; j < 32; j += 4) { acc[0] += v[j]; acc[1] += v[j + 1]; acc[2] += v[j + 2]; acc[3] += v[j + 3]; }
+      };
       for (int c0 = 0; c0 < rs32; c0 += 256) {
         const int nc = min(256, rs32 - c0);
         ptx::mbar_wait(&t_full[as], aph);
         ptx::tc_fence_after();
-        // this warp's 32-column blocks b0, b0+64, ...: the next block's TMEM load is in flight while
+        // this warp's 32-column blocks (every other one): the next block's TMEM load is in flight while
         // the current one goes through the MUFU pipe
-        const uint32_t tbase = tmem_base + (uint32_t(lg * 32) << 16) + as * 256;
-        float v[2][32];
-        int b0 = half * 32, cur_buf = 0;
-        if (b0 < nc) ptx::tmem_ld32(tbase + b0, v[0]);
-        for (; b0 < nc; b0 += 64) {
+        const uint32_t tbase = tmem_base + (uint32_t(lg * 32) << 16) + as * 256 + half * 32;
+        const int nb = (nc - half * 32 + 63) / 64;
+        float vA[32], vB[32];
+        if (nb > 0) ptx::tmem_ld32(tbase, vA);
+        for (int k = 0; k < nb; k += 2) {
           ptx::tmem_ld_wait();
-          if (b0 + 64 < nc) ptx::tmem_ld32(tbase + b0 + 64, v[cur_buf ^ 1]);
-          const float4* c4 = reinterpret_cast<const float4*>(s.c + c0 + b0);
-          const float* vv = v[cur_buf];
-#pragma unroll
-          for (int j = 0; j < 8; ++j) {
-            const float4 c = c4[j];
-            acc += fast_exp2(fmaf(vv[4 * j], a.scale_log2, -c.x));
-            acc2 += fast_exp2(fmaf(vv[4 * j + 1], a.scale_log2, -c.y));
-            acc += fast_exp2(fmaf(vv[4 * j + 2], a.scale_log2, -c.z));
-            acc2 += fast_exp2(fmaf(vv[4 * j + 3], a.scale_log2, -c.w));
+          if (k + 1 < nb) ptx::tmem_ld32(tbase + (k + 1) * 64, vB);
+          fold(vA, c0 + half * 32 + k * 64);
+          if (k + 1 < nb) {
+            ptx::tmem_ld_wait();
+            if (k + 2 < nb) ptx::tmem_ld32(tbase + (k + 2) * 64, vA);
+            fold(vB, c0 + half * 32 + (k + 1) * 64);
           }
-          cur_buf ^= 1;
         }
         ptx::tc_fence_before();
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(&t_empty[as]);
         if (++as == 2) { as = 0; aph ^= 1; }
       }
-      // merge the two column halves and store W's per-(KV head, super-chunk) column sum of this token
-      acc += acc2;
-      if (half == 1) acc_x[tok_in_tile] = acc;
-      ptx::named_bar_sync(2, 256);
+      // merge the two column halves (one 64-thread barrier per lane quarter, double-buffered exchange)
+      // and store W's per-(KV head, super-chunk) column sum of this token
+      const float mine = (acc[0] + acc[1]) + (acc[2] + acc[3]);
+      const int par = int(u & 1);
+      if (half == 1) acc_x[par][tok_in_tile] = mine;
+      ptx::named_bar_sync(2 + lg, 64);
       if (half == 0) {
         const int tok = t * TN + tok_in_tile;
         if (tok < a.Tn)
-          a.g.colsum[(size_t(gr.bl) * a.g.n_vh_max + gr.kvh * a.n_sc + gr.sc) * a.g.cap + tok] = acc + acc_x[tok_in_tile];
+          a.g.colsum[(size_t(gr.bl) * a.g.n_vh_max + gr.kvh * a.n_sc + gr.sc) * a.g.cap + tok] = mine + acc_x[par][tok_in_tile];
       }
-      ptx::named_bar_sync(2, 256);
     }
   }
   ptx::tc_fence_before();

@@ -10,6 +10,12 @@
 
 namespace hk {
 
+#ifdef HERMES_SELECT_TIMING
+#define SEL_T(n) do { __syncthreads(); if (blockIdx.x == 5 && threadIdx.x == 0) tstamp[n] = clock64(); } while (0)
+#else
+#define SEL_T(n)
+#endif
+
 constexpr int kSelThreads = 1024;
 constexpr int kBitmapWords = 2048;                   // 65536 coordinate values per axis
 
@@ -73,71 +79,110 @@ __device__ inline int block_reduce_min_i(int v, int* scratch) {
   return r;
 }
 
-// W of one layer at token i: per-KV-head column sums added in fixed head order, / (Hq * P).
-__device__ inline float mean_w(const Geom& g, int bl, int i, float inv_rows, int n_vh) {
-  const float* c = g.colsum + size_t(bl) * g.n_vh_max * g.cap + i;
+// a2 (first half), fully parallel: W_i = per-(KV head, super-chunk) column sums added in fixed order /
+// (Hq * P), and the per-layer max of W (order-independent, so an atomic max keeps it deterministic).
+__global__ void __launch_bounds__(256)
+k_wsum(Geom g, int Tn, int P, int n_vh) {
+  __shared__ float red[8];
+  const int Ls = g.L - g.n_shallow;
+  const int bl = (blockIdx.y / Ls) * g.L + g.n_shallow + blockIdx.y % Ls;
+  const int i = blockIdx.x * 256 + threadIdx.x;
   float w = 0.f;
-  for (int h = 0; h < n_vh; ++h) w += c[size_t(h) * g.cap];
-  return w * inv_rows;
+  if (i < Tn) {
+    const float* c = g.colsum + size_t(bl) * g.n_vh_max * g.cap + i;
+    for (int h = 0; h < n_vh; ++h) w += c[size_t(h) * g.cap];
+    w *= 1.0f / float(g.Hq * P);
+    g.wsum[size_t(bl) * g.cap + i] = w;
+  }
+  const float m = warp_max(w);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    float r = threadIdx.x < 8 ? red[threadIdx.x] : 0.f;
+    r = warp_max(r);
+    if (threadIdx.x == 0) atomicMax(&g.wmax[bl], __float_as_uint(r));
+  }
 }
 
 __global__ void __launch_bounds__(kSelThreads)
-k_select(Geom g, int cur, int Tn, int P, float k_forget, int norm_sum, float r_norm_sum, int n_vh) {
+k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum) {
   extern __shared__ float s_sc[];                    // [Tn] smoothed scores
-  __shared__ int hist[256];
+  // per-warp digit histograms (radix phase); the M-RoPE rank bitmap + word prefixes reuse the space later
+  __shared__ __align__(16) int whist[32 * 256];
+  __shared__ int part[4][256];
   __shared__ int warp_tot[33];
   __shared__ float red_f[32];
   __shared__ int red_i[32];
-  __shared__ uint32_t bitmap[kBitmapWords];
-  __shared__ int word_prefix[kBitmapWords];
   __shared__ uint32_t sel_prefix;
   __shared__ int sel_remaining;
+  uint32_t* bitmap = reinterpret_cast<uint32_t*>(whist);              // [kBitmapWords]
+  int* word_prefix = whist + kBitmapWords;                            // [kBitmapWords]
 
+#ifdef HERMES_SELECT_TIMING
+  __shared__ long long tstamp[8];
+#endif
+  SEL_T(0);
   const int bl = blockIdx.x, l = bl % g.L;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const bool scored0 = l >= g.n_shallow;
   const bool has_next = l + 1 < g.L;
   const bool scored1 = has_next && (l + 1 >= g.n_shallow);
-  const float inv_rows = 1.0f / float(g.Hq * P);
 
   // ---- a2: per-layer normalisation factor alpha (max or sum of W) ------------------------------
-  float n0 = 0.f, n1 = 0.f;
-  for (int i = tid; i < Tn; i += kSelThreads) {
-    if (scored0) { const float w = mean_w(g, bl, i, inv_rows, n_vh); n0 = norm_sum ? n0 + w : fmaxf(n0, w); }
-    if (scored1) { const float w = mean_w(g, bl + 1, i, inv_rows, n_vh); n1 = norm_sum ? n1 + w : fmaxf(n1, w); }
+  const float* w0 = g.wsum + size_t(bl) * g.cap;
+  const float* w1 = w0 + g.cap;
+  float n0, n1;
+  if (norm_sum) {
+    float t0 = 0.f, t1 = 0.f;
+    for (int i = tid; i < Tn; i += kSelThreads) { if (scored0) t0 += w0[i]; if (scored1) t1 += w1[i]; }
+    n0 = block_reduce_sum(t0, red_f);
+    n1 = block_reduce_sum(t1, red_f);
+  } else {
+    n0 = scored0 ? __uint_as_float(g.wmax[bl]) : 1.f;
+    n1 = scored1 ? __uint_as_float(g.wmax[bl + 1]) : 1.f;
   }
-  n0 = norm_sum ? block_reduce_sum(n0, red_f) : block_reduce_max(n0, red_f);
-  n1 = norm_sum ? block_reduce_sum(n1, red_f) : block_reduce_max(n1, red_f);
   const float a0 = scored0 ? 1.0f / n0 : 0.f, a1 = scored1 ? 1.0f / n1 : 0.f;
   const float om0 = g.omega[l], om1 = has_next ? g.omega[l + 1] : 0.f;
   const float lam = has_next ? g.lambda[l] : 0.f;
   const float r_norm = norm_sum ? r_norm_sum : 1.0f;
 
-  // ---- a2/a3: S^l, S^{l+1}, S~^l ---------------------------------------------------------------
+  SEL_T(1);
+  // ---- a2/a3: S^l, S^{l+1}, S~^l (4 tokens per thread per trip: all loads issued before use) ----
   float* scores_out = g.scores + size_t(bl) * g.cap;
-  for (int i = tid; i < Tn; i += kSelThreads) {
-    const float R = expf(-k_forget * float(Tn - 1 - i)) * r_norm;           // Eq. 1
-    const float A0 = scored0 ? mean_w(g, bl, i, inv_rows, n_vh) * a0 : 0.f;       // Eq. 2
-    float s = (1.0f - om0) * A0 + om0 * R;                                   // Eq. 4
-    if (has_next) {
-      const float A1 = scored1 ? mean_w(g, bl + 1, i, inv_rows, n_vh) * a1 : 0.f;
-      const float s1 = (1.0f - om1) * A1 + om1 * R;
-      s = (1.0f - lam) * s + lam * s1;                                       // Eq. 5
+  for (int i0 = tid; i0 < Tn; i0 += 4 * kSelThreads) {
+    float x0[4], x1[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const int i = i0 + j * kSelThreads;
+      x0[j] = (scored0 && i < Tn) ? w0[i] : 0.f;
+      x1[j] = (scored1 && i < Tn) ? w1[i] : 0.f;
     }
-    s_sc[i] = s;
-    scores_out[i] = s;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const int i = i0 + j * kSelThreads;
+      if (i < Tn) {
+        const float R = expf(-k_forget * float(Tn - 1 - i)) * r_norm;        // Eq. 1
+        float sc = (1.0f - om0) * (x0[j] * a0) + om0 * R;                    // Eq. 2, Eq. 4
+        if (has_next) {
+          const float s1 = (1.0f - om1) * (x1[j] * a1) + om1 * R;
+          sc = (1.0f - lam) * sc + lam * s1;                                 // Eq. 5
+        }
+        s_sc[i] = sc;
+        scores_out[i] = sc;
+      }
+    }
   }
+  if (tid == 0) { sel_prefix = 0u; sel_remaining = Tn - g.budget; }
+  for (int i = tid; i < 32 * 256; i += kSelThreads) whist[i] = 0;
   __syncthreads();
 
+  SEL_T(2);
   // ---- a4: radix select of the E-th smallest key (8 bits per round, MSB first) ------------------
-  const int E = Tn - g.budget;
-  if (tid == 0) { sel_prefix = 0u; sel_remaining = E; }
   for (int round = 0; round < 4; ++round) {
     const int shift = 24 - 8 * round;
     const uint32_t himask = round == 0 ? 0u : (0xFFFFFFFFu << (shift + 8));
-    if (tid < 256) hist[tid] = 0;
-    __syncthreads();
     const uint32_t prefix = sel_prefix;
+    int* my_hist = whist + warp * 256;
     for (int i0 = 0; i0 < Tn; i0 += kSelThreads) {     // whole warps iterate together
       const int i = i0 + tid;
       uint32_t digit = 0xFFFFFFFFu;
@@ -145,14 +190,26 @@ k_select(Geom g, int cur, int Tn, int P, float k_forget, int norm_sum, float r_n
         const uint32_t key = orderable(s_sc[i]);
         if ((key & himask) == prefix) digit = (key >> shift) & 255u;
       }
-      const uint32_t peers = __match_any_sync(0xffffffffu, digit);            // warp-aggregated histogram
-      if (digit != 0xFFFFFFFFu && lane == __ffs(peers) - 1) atomicAdd(&hist[digit], __popc(peers));
+      // warp-private histogram: the shared-memory atomics only ever collide inside one warp
+      if (digit != 0xFFFFFFFFu) atomicAdd(&my_hist[digit], 1);
+    }
+    __syncthreads();
+    {                                                   // fold 8 warp histograms per thread (4 partial sums per digit),
+      const int q = tid >> 8, d = tid & 255;            // clearing them for the next round
+      int c = 0;
+#pragma unroll
+      for (int w = 0; w < 8; ++w) { c += whist[(q * 8 + w) * 256 + d]; whist[(q * 8 + w) * 256 + d] = 0; }
+      part[q][d] = c;
     }
     __syncthreads();
     if (warp == 0) {                                    // find the bucket holding the E-th smallest
       int c[8], tot = 0;
 #pragma unroll
-      for (int j = 0; j < 8; ++j) { c[j] = hist[lane * 8 + j]; tot += c[j]; }
+      for (int j = 0; j < 8; ++j) {
+        const int d = lane * 8 + j;
+        c[j] = (part[0][d] + part[1][d]) + (part[2][d] + part[3][d]);
+        tot += c[j];
+      }
       int inc = tot;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) {
@@ -175,46 +232,77 @@ k_select(Geom g, int cur, int Tn, int P, float k_forget, int norm_sum, float r_n
     }
     __syncthreads();
   }
+  SEL_T(3);
   const uint32_t vstar = sel_prefix;                    // key of the E-th smallest score
   const int r_eq = sel_remaining;                       // evicted among keys == vstar (smallest indices)
 
-  // ---- flags + scans: thread t owns the contiguous tokens [t*per, (t+1)*per) --------------------
-  const int per = (Tn + kSelThreads - 1) / kSelThreads;
-  const int i_beg = min(tid * per, Tn), i_end = min(i_beg + per, Tn);
-  int n_eq = 0;
-  for (int i = i_beg; i < i_end; ++i) n_eq += (orderable(s_sc[i]) == vstar);
-  int tot_eq;
-  int eq_before = block_exscan(n_eq, warp_tot, &tot_eq);
-  int n_keep = 0;
-  for (int i = i_beg; i < i_end; ++i) {
-    const uint32_t key = orderable(s_sc[i]);
-    const bool evict = key < vstar || (key == vstar && eq_before < r_eq);
-    eq_before += (key == vstar);
-    n_keep += !evict;
+  // ---- flags + one packed scan over 32-token chunks; outputs are written coalesced -------------
+  // evicted(i) = key < v*  or  (key == v* and fewer than r_eq equal keys precede i)
+  // chunk c = tokens [32c, 32c+32): cnt_c = #(key < v*) | #(key == v*) << 16, exclusive-scanned over c.
+  const int n_chunks = (Tn + 31) >> 5;                                   // <= 1024 * kChunkPerThread
+  int* chunk_pre = whist;                                                // reuse: [n_chunks] packed prefixes
+  SEL_T(4);
+  for (int c = warp; c < n_chunks; c += 32) {
+    const int i = c * 32 + lane;
+    const uint32_t key = i < Tn ? orderable(s_sc[i]) : 0xFFFFFFFFu;
+    const uint32_t lt = __ballot_sync(0xffffffffu, i < Tn && key < vstar);
+    const uint32_t eq = __ballot_sync(0xffffffffu, i < Tn && key == vstar);
+    if (lane == 0) chunk_pre[c] = __popc(lt) | (__popc(eq) << 16);
   }
-  int tot_keep;
-  int out = block_exscan(n_keep, warp_tot, &tot_keep);
+  __syncthreads();
+  {
+    const int cpt = (n_chunks + kSelThreads - 1) / kSelThreads;          // chunks per thread (1 up to 32K tokens)
+    const int c_beg = min(tid * cpt, n_chunks), c_end = min(c_beg + cpt, n_chunks);
+    int mine = 0;
+    for (int c = c_beg; c < c_end; ++c) mine += chunk_pre[c];
+    int tot;
+    int run = block_exscan(mine, warp_tot, &tot);                        // both halves stay < 65536
+    for (int c = c_beg; c < c_end; ++c) { const int v = chunk_pre[c]; chunk_pre[c] = run; run += v; }
+  }
+  __syncthreads();
+  SEL_T(6);
   int32_t* kept = g.kept + size_t(bl) * g.budget;
-  eq_before = block_exscan(n_eq, warp_tot, &tot_eq);    // recompute the prefix consumed above
-  for (int i = i_beg; i < i_end; ++i) {
-    const uint32_t key = orderable(s_sc[i]);
-    const bool evict = key < vstar || (key == vstar && eq_before < r_eq);
-    eq_before += (key == vstar);
-    if (!evict) kept[out++] = i;
-  }
-  __syncthreads();                                      // kept[] visible to the whole block
-
-  // ---- a6: new positions into the other buffer ---------------------------------------------------
   const int32_t* pos_old = g.posc + (size_t(bl) * 2 + cur) * g.n_axes * g.cap;
   int32_t* pos_new = g.posc + (size_t(bl) * 2 + (cur ^ 1)) * g.n_axes * g.cap;
-  if (g.n_axes == 1) {                                  // Eq. 8: positions increase with the index -> rank = slot
-    int32_t* dl = g.delta + size_t(bl) * g.budget;
-    for (int s = tid; s < g.budget; s += kSelThreads) {
-      pos_new[s] = g.pos_offset + s;
-      dl[s] = g.pos_offset + s - pos_old[kept[s]];
+  int32_t* dl1 = g.delta + size_t(bl) * g.n_axes * g.budget;
+  const uint32_t lane_lt = (1u << lane) - 1u;
+  for (int cb = warp; cb < n_chunks; cb += 32 * 8) {                     // 8 chunks per trip: old positions first
+    int p_old[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const int i = (cb + 32 * j) * 32 + lane;
+      p_old[j] = (g.n_axes == 1 && i < Tn) ? pos_old[i] : 0;
     }
-    return;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const int c = cb + 32 * j;                                         // warp-uniform
+      if (c >= n_chunks) break;
+      const int i = c * 32 + lane;
+      const uint32_t key = i < Tn ? orderable(s_sc[i]) : 0xFFFFFFFFu;
+      const uint32_t lt = __ballot_sync(0xffffffffu, i < Tn && key < vstar);
+      const uint32_t eq = __ballot_sync(0xffffffffu, i < Tn && key == vstar);
+      const int pre = chunk_pre[c];
+      const int lt_before = (pre & 0xFFFF) + __popc(lt & lane_lt);
+      const int eq_before = (pre >> 16) + __popc(eq & lane_lt);
+      const bool evict = key < vstar || (key == vstar && eq_before < r_eq);
+      if (i < Tn && !evict) {
+        const int out = i - lt_before - min(eq_before, r_eq);            // slot of token i among the kept
+        kept[out] = i;
+        if (g.n_axes == 1) {                                             // Eq. 8: positions rise with the index -> rank = slot
+          pos_new[out] = g.pos_offset + out;
+          dl1[out] = g.pos_offset + out - p_old[j];
+        }
+      }
+    }
   }
+#ifdef HERMES_SELECT_TIMING
+  SEL_T(5);
+  if (blockIdx.x == 5 && threadIdx.x == 0) printf("select phases (cycles): setup %lld scores %lld radix %lld count+scan %lld write %lld\n", tstamp[1]-tstamp[0], tstamp[2]-tstamp[1], tstamp[3]-tstamp[2], tstamp[6]-tstamp[4], tstamp[5]-tstamp[6]);
+#endif
+  if (g.n_axes == 1) return;
+  __syncthreads();                                      // kept[] visible to the whole block
+
+  // ---- a6 (M-RoPE): per-axis rank among the distinct retained coordinates (Eq. 11) ----------------
   for (int a = 0; a < 3; ++a) {
     const int32_t* po = pos_old + size_t(a) * g.cap;
     int32_t* pn = pos_new + size_t(a) * g.cap;
@@ -235,6 +323,7 @@ k_select(Geom g, int cur, int Tn, int P, float k_forget, int norm_sum, float r_n
       for (int s = tid; s < g.budget; s += kSelThreads) { pn[s] = po[kept[s]]; dl[s] = 0; }
       continue;
     }
+    __syncthreads();
     for (int w = tid; w < kBitmapWords; w += kSelThreads) bitmap[w] = 0u;
     __syncthreads();
     for (int s = tid; s < g.budget; s += kSelThreads) {
@@ -244,11 +333,11 @@ k_select(Geom g, int cur, int Tn, int P, float k_forget, int norm_sum, float r_n
     __syncthreads();
     const int pc = __popc(bitmap[2 * tid]) + __popc(bitmap[2 * tid + 1]);   // 2 words per thread
     int tot;
-    const int pre = block_exscan(pc, warp_tot, &tot);
-    word_prefix[2 * tid] = pre;
-    word_prefix[2 * tid + 1] = pre + __popc(bitmap[2 * tid]);
+    const int wpre = block_exscan(pc, warp_tot, &tot);
+    word_prefix[2 * tid] = wpre;
+    word_prefix[2 * tid + 1] = wpre + __popc(bitmap[2 * tid]);
     __syncthreads();
-    for (int s = tid; s < g.budget; s += kSelThreads) {  // Eq. 11: offset + rank among distinct coordinates
+    for (int s = tid; s < g.budget; s += kSelThreads) {
       const int v = po[kept[s]] - vmin;
       const int p_new = g.pos_offset + word_prefix[v >> 5] + __popc(bitmap[v >> 5] & ((1u << (v & 31)) - 1u));
       pn[s] = p_new;
