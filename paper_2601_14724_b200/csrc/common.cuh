@@ -31,7 +31,7 @@ struct Geom {
   float* wsum;      // [B*L][cap] W_i: column sums added over KV heads / (Hq*P)  (Eq. 2)
   uint32_t* wmax;   // [B*L] max_i W_i as float bits (W >= 0), zeroed by k_append
   float* rowstat;   // [B*L][Hq*p_max][2] (m2, 1/Z) per probe row, log2 domain
-  float* partial;   // [B*L][Hq*p_max][n_part_max][2] partial (m2, z)
+  float* partial;   // partial (m2, z) of pass 1: SIMT path [B*L][Hq*p_max][n_part][2]; tcgen05 path [B*L][n_slot][Hq*p_max][2]
   float* scores;    // [B*L][cap]  smoothed scores S~ of the last eviction (a3)
   int32_t* kept;    // [B*L][budget] ascending kept indices I_l (a4)
   int32_t* delta;   // [B*L][n_axes][budget] p_new - p_old of every kept token (a6 -> a7)

@@ -68,7 +68,7 @@ inline Layout make_layout(const hermes_config& c) {
   y.esize = c.dtype == HERMES_BF16 ? 2 : 4;
   y.row_bytes = size_t(c.n_kv_heads) * c.head_dim * y.esize;
   y.n_part_max = (y.cap + 127) / 128;
-  y.n_vh_max = c.n_kv_heads * std::max(1, (c.n_q_heads / c.n_kv_heads * c.max_probe_tokens + 511) / 512);
+  y.n_vh_max = 4 * c.n_kv_heads * std::max(1, (c.n_q_heads / c.n_kv_heads * c.max_probe_tokens + 511) / 512);
   int ns = c.n_shallow, nd = c.n_deep;
   stage_split(c.n_layers, ns, nd);
   y.n_shallow = ns; y.n_deep = nd; y.n_middle = c.n_layers - ns - nd;

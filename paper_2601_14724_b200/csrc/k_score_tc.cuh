@@ -4,388 +4,439 @@
 // warp-specialised tcgen05 kernel fed by TMA, with fp32 accumulators in TMEM:
 //   pass 1 k_tc_stats  : D[row, tok] = Q_blk K_tile^T, probe rows on TMEM lanes -> each thread owns one
 //                        probe row and keeps its running (max, sum exp2) over the tokens: no cross-lane work.
-//   combine            : per probe row c_r = m_r + log2 Z_r.
 //   pass 2 k_tc_colsum : D[tok, row] = K_tile Q^T, tokens on TMEM lanes -> each thread owns one token and
-//                        accumulates sum_r exp2(s * scale - c_r): again no cross-lane work.
+//                        accumulates sum_r exp2(s * scale - c_r), c_r = m_r + log2 Z_r merged from pass 1.
 // A "group" = (stream, scored layer, KV head, row super-chunk of <= 512 probe rows); its Q rows stay in
-// shared memory while the K tiles of the group stream through a TMA ring.  The flattened (group, tile)
-// space is cut into equal contiguous ranges, one per CTA (<= #SM CTAs, 1 CTA/SM).
+// shared memory while the 128-token K tiles of the group stream through a TMA ring.  The flattened
+// (group, tile) space is cut into equal contiguous ranges, one per CTA (<= #SM CTAs, 1 CTA/SM).
+//
+// Both passes are bound by the exp2 rate of the XU pipe (16 results / clk / SM), and every MUFU, TMEM
+// load and mbarrier poll of an SM sub-partition shares one in-order MIO queue.  Hence the shape of the
+// epilogue: 16 warps (4 per sub-partition), each working through 32-column blocks with the TMEM load of
+// the NEXT block (and the barrier poll it may need) issued before the exp2 burst of the current one, and
+// no integer division (I2F / MUFU.RCP would queue behind the exp2 traffic) anywhere in a loop.
 #pragma once
 #include "host_state.cuh"
 #include "tc_ptx.cuh"
 
 namespace hk {
 
-constexpr int kTcRowsMax = 512;                 // probe rows resident per group (Q tile = 128 KB)
-constexpr int kTcQHalfBytes = kTcRowsMax * 128; // one 64-column half of the Q tile
-constexpr int kTcKBytes = 64 * 1024;            // K ring: 4 x 16 KB (pass 1) or 2 x 32 KB (pass 2)
-constexpr int kTcSmemBytes = 2 * kTcQHalfBytes + kTcKBytes + kTcRowsMax * 4 + 512 + 1024;
-constexpr int kTcStatsThreads = 64 + 8 * 32;    // producer, MMA, 8 epilogue warps
-constexpr int kTcColsumThreads = 64 + 8 * 32;   // producer, MMA, 8 epilogue warps
-constexpr int kTcSegTiles = 8;                  // pass 1: 64-token tiles per segment (one partial per segment,
-                                                // so the merge order never depends on the CTA schedule)
+constexpr int kTcRowsMax = 512;                 // probe rows resident per group (Q tile <= 128 KB)
+constexpr int kTcTile = 128;                    // tokens per K tile (both passes)
+constexpr int kTcKStage = kTcTile * 256;        // bytes per K tile: 128 tokens x 128 dims bf16
+constexpr int kTcKStagesMax = 4;                // K ring depth: as many 32 KB stages as fit beside the Q rows
+constexpr int kTcSmemMax = 232448;              // 227 KB dynamic shared memory per CTA
+constexpr int kTcEpiWarps = 16;                 // epilogue warps: 4 per SM sub-partition / TMEM lane quarter
+constexpr int kTcThreads = 64 + kTcEpiWarps * 32;   // producer, MMA, epilogue
+constexpr int kTcSegTiles = 4;                  // pass 1: 128-token tiles per segment (one partial pair per
+                                                // segment, so the merge order never depends on the CTA schedule)
 
 struct TcArgs {
   Geom g;
   int cur, Tn, P;
   float scale_log2;
   int R, RS, n_sc;          // probe rows per KV head (G*P), rows per super-chunk, super-chunks per KV head
-  int tpg;                  // token tiles per group (64-token tiles in pass 1, 128-token tiles in pass 2)
+  int tpg;                  // 128-token tiles per group
   int n_groups;             // B * Ls * Hkv * n_sc
-  int spg;                  // pass 1: 512-token segments per group = partial (m, z) slots per probe row
+  int spg;                  // pass 1: 512-token segments per group; partial (m, z) slots per probe row = 2 * spg
+  int q_half_bytes;         // shared-memory bytes of one 64-column half of the group's Q rows (64-row boxes)
+  int n_kst;                // K ring stages
+  long long* trace;         // optional event trace of CTA 0 (HERMES_TC_TRACE; NULL in production)
 };
 
-// ---- schedule: CTA c owns flattened units [c*U/nC, (c+1)*U/nC) -----------------------------------
-__host__ __device__ inline long long tc_unit_begin(long long U, int n_cta, int c) { return (U * c) / n_cta; }
-__host__ __device__ inline int tc_cta_of_unit(long long U, int n_cta, long long u) { return int(((u + 1) * n_cta - 1) / U); }
+// Event trace (diagnostics only): role 0 producer, 1 MMA issuer, 2 / 3 first / last epilogue warp.
+constexpr int kTcTraceN = 1024;
+constexpr int kTcTraceStride = 4 * kTcTraceN + 512;   // per kernel: 4 roles of CTA 0 + (start, end) globaltimer of every CTA
+#define TC_TRACE(role, id)                                                              \
+  do {                                                                                  \
+    if (kTrace && a.trace != nullptr && blockIdx.x == 0 && trace_n < kTcTraceN)         \
+      a.trace[(role) * kTcTraceN + trace_n++] = (clock64() << 4) | (id);                \
+  } while (0)
 
-struct TcGroup { int bl, kvh, sc, rs_valid, stat_row0; long long q_row0; };
-__device__ inline TcGroup tc_group(const TcArgs& a, int gi) {
-  TcGroup r;
-  const Geom& g = a.g;
-  const int Ls = g.L - g.n_shallow;
-  r.sc = gi % a.n_sc;
-  r.kvh = (gi / a.n_sc) % g.Hkv;
-  const int bls = gi / (a.n_sc * g.Hkv);
-  r.bl = (bls / Ls) * g.L + g.n_shallow + bls % Ls;
-  r.rs_valid = min(a.RS, a.R - r.sc * a.RS);
-  r.stat_row0 = r.kvh * a.R + r.sc * a.RS;
-  r.q_row0 = (long long)r.bl * g.Hq * a.P + r.stat_row0;
-  return r;
-}
+// ---- schedule: CTA c owns flattened units [c*U/nC, (c+1)*U/nC) -----------------------------------
+__host__ __device__ inline int tc_unit_begin(int U, int n_cta, int c) { return int(((long long)U * c) / n_cta); }
+
+// Group coordinates (super-chunk, KV head, scored layer, stream), advanced without integer division.
+struct TcCursor {
+  int sc, kvh, ls, bq;
+  __device__ inline void init(const TcArgs& a, int gi) {
+    const int Ls = a.g.L - a.g.n_shallow;
+    sc = gi % a.n_sc;
+    kvh = (gi / a.n_sc) % a.g.Hkv;
+    const int bls = gi / (a.n_sc * a.g.Hkv);
+    ls = bls % Ls; bq = bls / Ls;
+  }
+  __device__ inline void next(const TcArgs& a) {
+    if (++sc == a.n_sc) { sc = 0; if (++kvh == a.g.Hkv) { kvh = 0; if (++ls == a.g.L - a.g.n_shallow) { ls = 0; ++bq; } } }
+  }
+  __device__ inline int bl(const TcArgs& a) const { return bq * a.g.L + a.g.n_shallow + ls; }
+  __device__ inline int rs_valid(const TcArgs& a) const { return min(a.RS, a.R - sc * a.RS); }
+  __device__ inline int stat_row0(const TcArgs& a) const { return kvh * a.R + sc * a.RS; }
+};
 
 struct TcSmem {
-  uint8_t* q;        // [2 halves][512 rows][128 B], 128B-swizzled
-  uint8_t* k;        // K ring
+  uint8_t* q;        // [2 halves][q_half_bytes / 128 rows][128 B], 128B-swizzled
+  uint8_t* k;        // K ring: [stage][2 halves][128 tokens][128 B]
   float* c;          // [512] per-row c_r (pass 2)
   uint64_t* bars;    // mbarriers
   uint32_t* tmem;    // TMEM base address written by tcgen05.alloc
 };
-__device__ inline TcSmem tc_carve(uint8_t* raw) {
+__host__ __device__ inline int tc_smem_bytes(int q_half_bytes, int n_kst) {
+  return 1024 + 2 * q_half_bytes + n_kst * kTcKStage + kTcRowsMax * 4 + 256 + 16;
+}
+__device__ inline TcSmem tc_carve(uint8_t* raw, const TcArgs& a) {
   uint8_t* p = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(raw) + 1023) & ~uintptr_t(1023));
   TcSmem s;
-  s.q = p; p += 2 * kTcQHalfBytes;
-  s.k = p; p += kTcKBytes;
+  s.q = p; p += 2 * a.q_half_bytes;
+  s.k = p; p += a.n_kst * kTcKStage;
   s.c = reinterpret_cast<float*>(p); p += kTcRowsMax * 4;
   s.bars = reinterpret_cast<uint64_t*>(p); p += 256;
   s.tmem = reinterpret_cast<uint32_t*>(p);
   return s;
 }
 
-// Loads the group's Q rows (both 64-column halves) in 64-row boxes.
-__device__ inline void tc_load_q(const TcSmem& s, const CUtensorMap* tq, uint64_t* bar, const TcGroup& gr) {
-  const int n_box = (gr.rs_valid + 63) / 64;
-  ptx::mbar_expect_tx(bar, uint32_t(n_box) * 2 * 8192);
-  for (int h = 0; h < 2; ++h)
-    for (int bx = 0; bx < n_box; ++bx)
-      ptx::tma_load_2d(s.q + h * kTcQHalfBytes + bx * 8192, tq, bar, h * 64, int(gr.q_row0) + bx * 64);
+struct TcBars {
+  uint64_t *k_full, *k_empty, *t_full, *t_empty, *q_full, *q_empty;
+};
+__device__ inline TcBars tc_bars(const TcSmem& s) {
+  TcBars b;
+  b.k_full = s.bars; b.k_empty = s.bars + kTcKStagesMax;
+  b.t_full = s.bars + 2 * kTcKStagesMax; b.t_empty = b.t_full + 2;
+  b.q_full = b.t_empty + 2; b.q_empty = b.q_full + 1;
+  return b;
 }
-
-// =====================================================================================================
-// pass 1: per probe row, partial (max, sum exp2) over this CTA's token range of the group
-// =====================================================================================================
-__global__ void __launch_bounds__(kTcStatsThreads, 1)
-k_tc_stats(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k, TcArgs a) {
-  extern __shared__ uint8_t smem_raw[];
-  const TcSmem s = tc_carve(smem_raw);
-  constexpr int NS = 4, TN = 64, KSTAGE = 16384;
-  uint64_t* k_full = s.bars;            // [NS]
-  uint64_t* k_empty = s.bars + NS;      // [NS]
-  uint64_t* t_full = s.bars + 2 * NS;   // [2]
-  uint64_t* t_empty = t_full + 2;       // [2]
-  uint64_t* q_full = t_empty + 2;
-  uint64_t* q_empty = q_full + 1;
+__device__ inline uint32_t tc_prologue(const TcSmem& s, const TcBars& b, const TcArgs& a, const CUtensorMap* tq, const CUtensorMap* tk) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const long long U = (long long)a.n_groups * a.spg;                     // schedule unit = (group, segment)
-  const int n_cta = gridDim.x, cta = blockIdx.x;
-  const long long s0 = tc_unit_begin(U, n_cta, cta), s1 = tc_unit_begin(U, n_cta, cta + 1);
-
   if (warp == 0 && lane == 0) {
-    ptx::prefetch_tmap(&tmap_q); ptx::prefetch_tmap(&tmap_k);
-    for (int i = 0; i < NS; ++i) { ptx::mbar_init(&k_full[i], 1); ptx::mbar_init(&k_empty[i], 1); }
-    for (int i = 0; i < 2; ++i) { ptx::mbar_init(&t_full[i], 1); ptx::mbar_init(&t_empty[i], 8); }
-    ptx::mbar_init(q_full, 1); ptx::mbar_init(q_empty, 1);
+    ptx::prefetch_tmap(tq); ptx::prefetch_tmap(tk);
+    for (int i = 0; i < a.n_kst; ++i) { ptx::mbar_init(&b.k_full[i], 1); ptx::mbar_init(&b.k_empty[i], 1); }
+    for (int i = 0; i < 2; ++i) { ptx::mbar_init(&b.t_full[i], 1); ptx::mbar_init(&b.t_empty[i], kTcEpiWarps); }
+    ptx::mbar_init(b.q_full, 1); ptx::mbar_init(b.q_empty, 1);
     ptx::fence_barrier_init();
   }
   if (warp == 1) ptx::tmem_alloc(s.tmem, 512);
   ptx::tc_fence_before();
   __syncthreads();
   ptx::tc_fence_after();
-  const uint32_t tmem_base = *s.tmem;
+  return *s.tmem;
+}
+
+// TMA producer (one thread), identical for both passes: the 128-token K tiles of units [u0, u1) and the
+// Q rows of each group the CTA touches (both 64-column halves, 64-row boxes).  kSeg: unit = (group,
+// segment of kTcSegTiles tiles); otherwise unit = (group, tile).  A new group's first K tile is requested
+// before the Q buffer is waited for, so it is in flight while the old group's MMAs drain.
+template <bool kSeg, bool kTrace>
+__device__ inline void tc_producer(const TcSmem& s, const TcBars& b, const CUtensorMap* tq, const CUtensorMap* tk,
+                                   const TcArgs& a, int u0, int u1) {
+  const int upg = kSeg ? a.spg : a.tpg;
+  int ks = 0, kph = 0, n_q = 0, trace_n = 0;
+  bool new_group = true;
+  int x = u0 % upg;
+  TcCursor g; g.init(a, u0 / upg);
+  for (int u = u0; u < u1; ++u) {
+    const int t0 = kSeg ? x * kTcSegTiles : x, t1 = kSeg ? min(a.tpg, t0 + kTcSegTiles) : x + 1;
+    const int bl = g.bl(a);
+    for (int t = t0; t < t1; ++t) {
+      ptx::mbar_wait(&b.k_empty[ks], kph ^ 1);
+      TC_TRACE(0, 1);
+      ptx::mbar_expect_tx(&b.k_full[ks], kTcKStage);
+      const int row = int((size_t(bl) * 2 + a.cur) * a.g.cap) + t * kTcTile;
+      for (int h = 0; h < 2; ++h)
+        for (int bx = 0; bx < 2; ++bx)
+          ptx::tma_load_2d(s.k + ks * kTcKStage + h * 16384 + bx * 8192, tk, &b.k_full[ks], g.kvh * 128 + h * 64, row + bx * 64);
+      if (++ks == a.n_kst) { ks = 0; kph ^= 1; }
+      if (new_group) {
+        if (n_q > 0) ptx::mbar_wait(b.q_empty, (n_q - 1) & 1);
+        TC_TRACE(0, 2);
+        const int n_box = (g.rs_valid(a) + 63) >> 6;
+        const int q_row0 = bl * a.g.Hq * a.P + g.stat_row0(a);
+        ptx::mbar_expect_tx(b.q_full, uint32_t(n_box) * 2 * 8192);
+        for (int h = 0; h < 2; ++h)
+          for (int bx = 0; bx < n_box; ++bx)
+            ptx::tma_load_2d(s.q + h * a.q_half_bytes + bx * 8192, tq, b.q_full, h * 64, q_row0 + bx * 64);
+        ++n_q; new_group = false;
+      }
+    }
+    if (++x == upg) { x = 0; g.next(a); new_group = true; }
+  }
+}
+
+// =====================================================================================================
+// pass 1: per probe row, partial (max, sum exp2) over this CTA's token range of the group.
+// D[row, tok] = Q_blk K_tile^T: probe rows on TMEM lanes, so every epilogue thread owns one probe row.
+// A TMEM stage (256 columns) holds a "half-group" = 2 row blocks x 128 tokens; epilogue warp
+// (row block rbl, 64-token half th, lane quarter lg) takes its 64 columns as two 32-column blocks.
+// =====================================================================================================
+template <int kVar, bool kTrace>
+__global__ void __launch_bounds__(kTcThreads, 1)
+k_tc_stats(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k, TcArgs a) {
+  extern __shared__ uint8_t smem_raw[];
+  const TcSmem s = tc_carve(smem_raw, a);
+  const TcBars b = tc_bars(s);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int U = a.n_groups * a.spg;                                      // schedule unit = (group, segment)
+  const int s0 = tc_unit_begin(U, gridDim.x, blockIdx.x), s1 = tc_unit_begin(U, gridDim.x, blockIdx.x + 1);
+  if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.trace[4 * kTcTraceN + 2 * blockIdx.x] = t; }
+  const uint32_t tmem_base = tc_prologue(s, b, a, &tmap_q, &tmap_k);
 
   if (warp == 0) {
-    // ---------------- TMA producer ----------------
-    if (lane == 0) {
-      int ks = 0, kph = 0, n_q = 0, prev = -1;
-      for (long long u = s0; u < s1; ++u) {
-        const int gi = int(u / a.spg), sg = int(u % a.spg);
-        const TcGroup gr = tc_group(a, gi);
-        if (gi != prev) {
-          if (n_q > 0) ptx::mbar_wait(q_empty, (n_q - 1) & 1);
-          tc_load_q(s, &tmap_q, q_full, gr);
-          ++n_q; prev = gi;
-        }
-        const int t_end = min(a.tpg, (sg + 1) * kTcSegTiles);
-        for (int t = sg * kTcSegTiles; t < t_end; ++t) {
-          ptx::mbar_wait(&k_empty[ks], kph ^ 1);
-          ptx::mbar_expect_tx(&k_full[ks], KSTAGE);
-          const int row = int((size_t(gr.bl) * 2 + a.cur) * a.g.cap) + t * TN;
-          for (int h = 0; h < 2; ++h)
-            ptx::tma_load_2d(s.k + ks * KSTAGE + h * 8192, &tmap_k, &k_full[ks], gr.kvh * 128 + h * 64, row);
-          if (++ks == NS) { ks = 0; kph ^= 1; }
-        }
-      }
-    }
+    if (lane == 0) tc_producer<true, kTrace>(s, b, &tmap_q, &tmap_k, a, s0, s1);
   } else if (warp == 1) {
-    // ---------------- MMA issuer ----------------
-    const uint32_t idesc = ptx::idesc_bf16_f32(128, TN);
-    int ks = 0, kph = 0, as = 0, aph = 0, n_q = 0, prev = -1, n_rb = 0;
-    for (long long u = s0; u < s1; ++u) {
-      const int gi = int(u / a.spg), sg = int(u % a.spg);
-      if (gi != prev) {
-        const TcGroup gr = tc_group(a, gi);
-        n_rb = (gr.rs_valid + 127) / 128;
-        ptx::mbar_wait(q_full, n_q & 1);
-        ++n_q; prev = gi;
-      }
-      const bool last_seg_of_group = (u + 1 == s1) || int((u + 1) / a.spg) != gi;
-      const int t_end = min(a.tpg, (sg + 1) * kTcSegTiles);
-      for (int t = sg * kTcSegTiles; t < t_end; ++t) {
-        ptx::mbar_wait(&k_full[ks], kph);
-        ptx::mbar_wait(&t_empty[as], aph ^ 1);
-        ptx::tc_fence_after();
-        if (lane == 0) {
-          for (int rb = 0; rb < n_rb; ++rb) {
+    // ---------------- MMA issuer: the whole warp runs the loop, one elected lane issues ----------------
+    const uint32_t idesc = ptx::idesc_bf16_f32(128, kTcTile);
+    const uint32_t q_lo = ptx::smem_desc_lo(ptx::smem_u32(s.q)), k_lo = ptx::smem_desc_lo(ptx::smem_u32(s.k));
+    const uint32_t q_half16 = uint32_t(a.q_half_bytes) >> 4;
+    int ks = 0, kph = 0, as = 0, aph = 0, n_q = 0, trace_n = 0;
+    bool new_group = true;
+    int x = s0 % a.spg;
+    TcCursor g; g.init(a, s0 / a.spg);
+    for (int u = s0; u < s1; ++u) {
+      const int n_rb = (g.rs_valid(a) + 127) >> 7;
+      if (new_group) { ptx::mbar_wait(b.q_full, n_q & 1); ++n_q; new_group = false; }
+      const bool last_seg_of_group = (u + 1 == s1) || x + 1 == a.spg;
+      const int t_end = min(a.tpg, (x + 1) * kTcSegTiles);
+      for (int t = x * kTcSegTiles; t < t_end; ++t) {
+        ptx::mbar_wait(&b.k_full[ks], kph);
+        if (lane == 0) TC_TRACE(1, 1);
+        const uint32_t kb_lo = k_lo + uint32_t(ks) * (kTcKStage >> 4);
+        for (int hg = 0; 2 * hg < n_rb; ++hg) {
+          ptx::mbar_wait(&b.t_empty[as], aph ^ 1);
+          ptx::tc_fence_after();
+          if (lane == 0) TC_TRACE(1, 2);
+          const uint32_t qa_lo = q_lo + uint32_t(2 * hg) * 1024u, d0 = tmem_base + as * 256;
+          const bool two = 2 * hg + 1 < n_rb;
+          if (ptx::elect_one()) {
 #pragma unroll
-            for (int kk = 0; kk < 8; ++kk) {
-              const int h = kk >> 2;
-              const uint64_t ad = ptx::smem_desc_sw128(ptx::smem_u32(s.q + h * kTcQHalfBytes + rb * 16384)) + uint64_t((kk & 3) * 2);
-              const uint64_t bd = ptx::smem_desc_sw128(ptx::smem_u32(s.k + ks * KSTAGE + h * 8192)) + uint64_t((kk & 3) * 2);
-              ptx::mma_bf16(tmem_base + as * 256 + rb * TN, ad, bd, idesc, kk > 0);
+            for (int kk = 0; kk < 8; ++kk)
+              ptx::mma_bf16_lohi(d0, qa_lo + (kk >> 2) * q_half16 + (kk & 3) * 2,
+                                 kb_lo + (kk >> 2) * 1024u + (kk & 3) * 2, ptx::kSmemDescHiSw128, idesc, kk > 0);
+            if (two) {
+#pragma unroll
+              for (int kk = 0; kk < 8; ++kk)
+                ptx::mma_bf16_lohi(d0 + kTcTile, qa_lo + 1024u + (kk >> 2) * q_half16 + (kk & 3) * 2,
+                                   kb_lo + (kk >> 2) * 1024u + (kk & 3) * 2, ptx::kSmemDescHiSw128, idesc, kk > 0);
             }
+            ptx::mma_commit(&b.t_full[as]);
           }
-          ptx::mma_commit(&k_empty[ks]);
-          ptx::mma_commit(&t_full[as]);
-          if (last_seg_of_group && t + 1 == t_end) ptx::mma_commit(q_empty);
+          __syncwarp();
+          if (lane == 0) TC_TRACE(1, 3);
+          if (++as == 2) { as = 0; aph ^= 1; }
+        }
+        if (ptx::elect_one()) {
+          ptx::mma_commit(&b.k_empty[ks]);
+          if (last_seg_of_group && t + 1 == t_end) ptx::mma_commit(b.q_empty);
         }
         __syncwarp();
-        if (++ks == NS) { ks = 0; kph ^= 1; }
-        if (++as == 2) { as = 0; aph ^= 1; }
+        if (++ks == a.n_kst) { ks = 0; kph ^= 1; }
       }
+      if (++x == a.spg) { x = 0; g.next(a); new_group = true; }
     }
   } else {
-    // ---------------- epilogue: two probe rows per thread (row blocks rb0, rb0+1), software-pipelined:
-    // the TMEM load of one row block is always in flight while the other goes through the MUFU pipe ----
-    const int e = warp - 2, rb0 = (e >> 2) * 2, lg = warp & 3;
-    int as = 0, aph = 0;
-    float m_run[2] = {-INFINITY, -INFINITY}, z[2] = {0.f, 0.f};
-    float vA[TN], vB[TN];
-    // running (max, sum exp2) of one row over one 64-token tile
-    auto fold = [&](float (&v)[TN], int t, float& m_r, float& z_r) {
-      const int n_valid = min(TN, a.Tn - t * TN);                       // ragged last tile of the group
-      if (n_valid < TN) {
+    // ---------------- epilogue: one probe row x 64 tokens per thread per stage ----------------
+    const int e = warp - 2, rbl = e >> 3, th = (e >> 2) & 1, lg = warp & 3;
+    const uint32_t t_addr = tmem_base + (uint32_t(lg * 32) << 16) + rbl * kTcTile + th * 64;
+    int as = 0, aph = 0, trace_n = 0;
+    const int trole = e == 0 ? 2 : 3;
+    const bool tr = kTrace && lane == 0 && (e == 0 || e == kTcEpiWarps - 1);
+    float m0 = -INFINITY, z0 = 0.f, m1 = -INFINITY, z1 = 0.f;            // running (max, sum) per half-group
+    float v[64];
+    // online (max, sum exp2) update with this thread's 64 tokens of one stage
+    auto fold = [&](int n_valid, float& m_run, float& z_run) {
+      if (n_valid < 64) {                                                // ragged last tile of the group
 #pragma unroll
-        for (int j = 0; j < TN; ++j) if (j >= n_valid) v[j] = -INFINITY;
+        for (int j = 0; j < 64; ++j) if (j >= n_valid) v[j] = -INFINITY;
       }
       float mx[4] = {v[0], v[1], v[2], v[3]};
 #pragma unroll
-      for (int j = 4; j < TN; j += 4) {
+      for (int j = 4; j < 64; j += 4) {
         mx[0] = fmaxf(mx[0], v[j]); mx[1] = fmaxf(mx[1], v[j + 1]);
         mx[2] = fmaxf(mx[2], v[j + 2]); mx[3] = fmaxf(mx[3], v[j + 3]);
       }
-      const float m_new = fmaxf(m_r, fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])) * a.scale_log2);
-#pragma unroll
-      for (int j = 0; j < TN; ++j) v[j] = fmaf(v[j], a.scale_log2, -m_new);
-#pragma unroll
-      for (int j = 0; j < TN; ++j) v[j] = fast_exp2(v[j]);
+      const float m_new = fmaxf(m_run, fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3])) * a.scale_log2);
       float sm[4] = {0.f, 0.f, 0.f, 0.f};
+      if (kVar & 1) {                                                    // FFMA / MUFU / FADD interleaved
 #pragma unroll
-      for (int j = 0; j < TN; j += 4) { sm[0] += v[j]; sm[1] += v[j + 1]; sm[2] += v[j + 2]; sm[3] += v[j + 3]; }
-      z_r = z_r * fast_exp2(m_r - m_new) + ((sm[0] + sm[1]) + (sm[2] + sm[3]));
-      m_r = m_new;
-    };
-    long long u = s0;
-    if (u < s1) {
-      int gi = int(u / a.spg), sg = int(u % a.spg);
-      TcGroup gr = tc_group(a, gi);
-      int t = sg * kTcSegTiles, t_end = min(a.tpg, t + kTcSegTiles);
-      bool act0 = rb0 * 128 + lg * 32 < gr.rs_valid, act1 = (rb0 + 1) * 128 + lg * 32 < gr.rs_valid;
-      const uint32_t lane_base = uint32_t(lg * 32) << 16;
-      ptx::mbar_wait(&t_full[as], aph);
-      ptx::tc_fence_after();
-      if (act0) { ptx::tmem_ld32(tmem_base + lane_base + as * 256 + rb0 * TN, vA); ptx::tmem_ld32(tmem_base + lane_base + as * 256 + rb0 * TN + 32, vA + 32); }
-      while (true) {
-        ptx::tmem_ld_wait();                                             // row block rb0 of tile t is in registers
-        if (act1) { ptx::tmem_ld32(tmem_base + lane_base + as * 256 + (rb0 + 1) * TN, vB); ptx::tmem_ld32(tmem_base + lane_base + as * 256 + (rb0 + 1) * TN + 32, vB + 32); }
-        if (act0) fold(vA, t, m_run[0], z[0]);
-        ptx::tmem_ld_wait();                                             // row block rb0+1 too: free the TMEM stage
-        ptx::tc_fence_before();
-        __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(&t_empty[as]);
-        if (++as == 2) { as = 0; aph ^= 1; }
-        // advance to the next tile of this CTA's range and start its first load
-        const int t_cur = t, sg_cur = sg;
-        const TcGroup gr_cur = gr;
-        const bool seg_done = t + 1 >= t_end, act1_cur = act1;
-        bool more = true;
-        if (!seg_done) { ++t; }
-        else if (++u < s1) {
-          const int gi_n = int(u / a.spg);
-          sg = int(u % a.spg);
-          if (gi_n != gi) { gi = gi_n; gr = tc_group(a, gi); }
-          t = sg * kTcSegTiles; t_end = min(a.tpg, t + kTcSegTiles);
-        } else more = false;
-        const bool act0_cur = act0;
-        if (more) {
-          act0 = rb0 * 128 + lg * 32 < gr.rs_valid; act1 = (rb0 + 1) * 128 + lg * 32 < gr.rs_valid;
-          ptx::mbar_wait(&t_full[as], aph);
-          ptx::tc_fence_after();
-          if (act0) { ptx::tmem_ld32(tmem_base + lane_base + as * 256 + rb0 * TN, vA); ptx::tmem_ld32(tmem_base + lane_base + as * 256 + rb0 * TN + 32, vA + 32); }
-        }
-        if (act1_cur) fold(vB, t_cur, m_run[1], z[1]);
-        if (seg_done) {                                                  // one partial per (row, segment)
+        for (int j = 0; j < 64; j += 4) {
 #pragma unroll
-          for (int k = 0; k < 2; ++k) {
-            const int row = (rb0 + k) * 128 + lg * 32 + lane;
-            if ((k == 0 ? act0_cur : act1_cur) && row < gr_cur.rs_valid) {
-              float* out = a.g.partial + ((size_t(gr_cur.bl) * a.g.Hq * a.g.p_max + gr_cur.stat_row0 + row) * a.spg + sg_cur) * 2;
-              out[0] = m_run[k]; out[1] = z[k];
-            }
-            m_run[k] = -INFINITY; z[k] = 0.f;
-          }
+          for (int i = 0; i < 4; ++i) sm[i] += fast_exp2(fmaf(v[j + i], a.scale_log2, -m_new));
         }
-        if (!more) break;
+      } else {                                                           // three phases
+#pragma unroll
+        for (int j = 0; j < 64; ++j) v[j] = fmaf(v[j], a.scale_log2, -m_new);
+#pragma unroll
+        for (int j = 0; j < 64; ++j) v[j] = fast_exp2(v[j]);
+#pragma unroll
+        for (int j = 0; j < 64; j += 4) { sm[0] += v[j]; sm[1] += v[j + 1]; sm[2] += v[j + 2]; sm[3] += v[j + 3]; }
       }
+      z_run = z_run * fast_exp2(m_run - m_new) + ((sm[0] + sm[1]) + (sm[2] + sm[3]));
+      m_run = m_new;
+    };
+    int x = s0 % a.spg;
+    TcCursor g; g.init(a, s0 / a.spg);
+    for (int u = s0; u < s1; ++u) {
+      const int rs_valid = g.rs_valid(a);
+      const bool two = rs_valid > 256;                                   // the group has a second half-group
+      const bool act0 = rbl * 128 + lg * 32 < rs_valid, act1 = (2 + rbl) * 128 + lg * 32 < rs_valid;
+      const int t_end = min(a.tpg, (x + 1) * kTcSegTiles);
+      for (int t = x * kTcSegTiles; t < t_end; ++t) {
+        const int n_valid = a.Tn - (t * kTcTile + th * 64);
+#pragma unroll
+        for (int hg = 0; hg < 2; ++hg) {
+          if (hg == 1 && !two) break;
+          const bool act = (hg == 0 ? act0 : act1) && n_valid > 0;
+          ptx::mbar_wait(&b.t_full[as], aph);
+          ptx::tc_fence_after();
+          if (tr) TC_TRACE(trole, 1);
+          if (act) {
+            ptx::tmem_ld32(t_addr + as * 256, v);
+            ptx::tmem_ld32(t_addr + as * 256 + 32, v + 32);
+            ptx::tmem_ld_wait();
+          }
+          ptx::tc_fence_before();
+          __syncwarp();
+          if (lane == 0) ptx::mbar_arrive(&b.t_empty[as]);               // accumulators are in registers
+          if (tr) TC_TRACE(trole, 2);
+          if (++as == 2) { as = 0; aph ^= 1; }
+          if (act) { if (hg == 0) fold(n_valid, m0, z0); else fold(n_valid, m1, z1); }
+          if (tr) TC_TRACE(trole, 3);
+        }
+      }
+      // segment done: one partial per (segment, token half, row); rows / halves that saw no token write (-inf, 0)
+      {
+        float2* part = reinterpret_cast<float2*>(a.g.partial) +
+                       (size_t(g.bl(a)) * (2 * a.spg) + 2 * x + th) * (a.g.Hq * a.g.p_max) + g.stat_row0(a);
+        const int row_a = rbl * 128 + lg * 32 + lane, row_b = row_a + 256;
+        if (row_a < rs_valid) part[row_a] = make_float2(m0, z0);
+        if (row_b < rs_valid) part[row_b] = make_float2(m1, z1);
+        m0 = m1 = -INFINITY; z0 = z1 = 0.f;
+      }
+      if (++x == a.spg) { x = 0; g.next(a); }
     }
   }
   ptx::tc_fence_before();
   __syncthreads();
+  if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.trace[4 * kTcTraceN + 2 * blockIdx.x + 1] = t; }
   if (warp == 1) ptx::tmem_dealloc(tmem_base, 512);
 }
 
+// Pass-2 group prologue: merges each probe row's per-(segment, half) (m, z) partials of pass 1 in slot
+// order into c_r = m_r + log2 Z_r (shared memory); rows past the group get +inf: exp2(-inf) = 0.
+// 16 independent loads in flight per thread.  Kept out of line so its registers do not weigh on the hot loop.
+__device__ __noinline__ void tc_merge_rows(const float2* pr, int n_slot, int rows_total, int rs_valid, float* c_out, int et) {
+  for (int i = et; i < kTcRowsMax; i += kTcEpiWarps * 32) {
+    float c = INFINITY;
+    if (i < rs_valid) {
+      const float2* p2 = pr + i;
+      float m = -INFINITY, zz = 0.f;
+      for (int j0 = 0; j0 < n_slot; j0 += 16) {
+        float2 pv[16];
+#pragma unroll
+        for (int j = 0; j < 16; ++j) pv[j] = __ldg(p2 + size_t(min(j0 + j, n_slot - 1)) * rows_total);   // always in range: no branch
+#pragma unroll
+        for (int j = 0; j < 16; ++j) if (j0 + j >= n_slot) pv[j] = make_float2(-INFINITY, 0.f);
+        float mc = m;
+#pragma unroll
+        for (int j = 0; j < 16; ++j) mc = fmaxf(mc, pv[j].x);
+        zz = m == -INFINITY ? 0.f : zz * fast_exp2(m - mc);
+#pragma unroll
+        for (int j = 0; j < 16; ++j) zz += pv[j].y * fast_exp2(pv[j].x - mc);
+        m = mc;
+      }
+      c = m + log2f(zz);
+    }
+    c_out[i] = c;
+  }
+}
+
 // =====================================================================================================
-// pass 2: per token, sum over the group's probe rows of exp2(s * scale - c_r)
+// pass 2: per token, sum over the group's probe rows of exp2(s * scale - c_r).
+// D[tok, row] = K_tile Q^T: tokens on TMEM lanes, so every epilogue thread owns one token; a TMEM stage
+// holds a chunk of <= 256 probe rows of the 128-token tile; epilogue warp (lane quarter lg, column
+// quarter cq) takes 32-column blocks cq and cq + 4 of the chunk.
 // =====================================================================================================
-__global__ void __launch_bounds__(kTcColsumThreads, 1)
+template <int kVar, bool kTrace>
+__global__ void __launch_bounds__(kTcThreads, 1)
 k_tc_colsum(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k, TcArgs a) {
   extern __shared__ uint8_t smem_raw[];
-  const TcSmem s = tc_carve(smem_raw);
-  constexpr int NS = 2, TN = 128, KSTAGE = 32768;
-  __shared__ float acc_x[2][128];       // partial sums of the upper column-half warps (double-buffered)
-  uint64_t* k_full = s.bars;            // [NS]
-  uint64_t* k_empty = s.bars + NS;      // [NS]
-  uint64_t* t_full = s.bars + 2 * NS;   // [2]
-  uint64_t* t_empty = t_full + 2;       // [2]
-  uint64_t* q_full = t_empty + 2;
-  uint64_t* q_empty = q_full + 1;
+  const TcSmem s = tc_carve(smem_raw, a);
+  const TcBars b = tc_bars(s);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const long long U = (long long)a.n_groups * a.tpg;
-  const int n_cta = gridDim.x, cta = blockIdx.x;
-  const long long u0 = tc_unit_begin(U, n_cta, cta), u1 = tc_unit_begin(U, n_cta, cta + 1);
-
-  if (warp == 0 && lane == 0) {
-    ptx::prefetch_tmap(&tmap_q); ptx::prefetch_tmap(&tmap_k);
-    for (int i = 0; i < NS; ++i) { ptx::mbar_init(&k_full[i], 1); ptx::mbar_init(&k_empty[i], 1); }
-    for (int i = 0; i < 2; ++i) { ptx::mbar_init(&t_full[i], 1); ptx::mbar_init(&t_empty[i], 8); }
-    ptx::mbar_init(q_full, 1); ptx::mbar_init(q_empty, 1);
-    ptx::fence_barrier_init();
-  }
-  if (warp == 1) ptx::tmem_alloc(s.tmem, 512);
-  ptx::tc_fence_before();
-  __syncthreads();
-  ptx::tc_fence_after();
-  const uint32_t tmem_base = *s.tmem;
+  const int U = a.n_groups * a.tpg;
+  const int u0 = tc_unit_begin(U, gridDim.x, blockIdx.x), u1 = tc_unit_begin(U, gridDim.x, blockIdx.x + 1);
+  if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.trace[4 * kTcTraceN + 2 * blockIdx.x] = t; }
+  const uint32_t tmem_base = tc_prologue(s, b, a, &tmap_q, &tmap_k);
 
   if (warp == 0) {
-    if (lane == 0) {
-      int ks = 0, kph = 0, n_q = 0, prev = -1;
-      for (long long u = u0; u < u1; ++u) {
-        const int gi = int(u / a.tpg), t = int(u % a.tpg);
-        const TcGroup gr = tc_group(a, gi);
-        if (gi != prev) {
-          if (n_q > 0) ptx::mbar_wait(q_empty, (n_q - 1) & 1);
-          tc_load_q(s, &tmap_q, q_full, gr);
-          ++n_q; prev = gi;
-        }
-        ptx::mbar_wait(&k_empty[ks], kph ^ 1);
-        ptx::mbar_expect_tx(&k_full[ks], KSTAGE);
-        const int row = int((size_t(gr.bl) * 2 + a.cur) * a.g.cap) + t * TN;
-        for (int h = 0; h < 2; ++h)
-          for (int bx = 0; bx < 2; ++bx)
-            ptx::tma_load_2d(s.k + ks * KSTAGE + h * 16384 + bx * 8192, &tmap_k, &k_full[ks], gr.kvh * 128 + h * 64, row + bx * 64);
-        if (++ks == NS) { ks = 0; kph ^= 1; }
-      }
-    }
+    if (lane == 0) tc_producer<false, kTrace>(s, b, &tmap_q, &tmap_k, a, u0, u1);
   } else if (warp == 1) {
-    int ks = 0, kph = 0, as = 0, aph = 0, n_q = 0, prev = -1, rs32 = 0;
-    for (long long u = u0; u < u1; ++u) {
-      const int gi = int(u / a.tpg);
-      if (gi != prev) {
-        const TcGroup gr = tc_group(a, gi);
-        rs32 = (gr.rs_valid + 31) & ~31;
-        ptx::mbar_wait(q_full, n_q & 1);
-        ++n_q; prev = gi;
-      }
-      ptx::mbar_wait(&k_full[ks], kph);
+    // ---------------- MMA issuer: the whole warp runs the loop, one elected lane issues ----------------
+    const uint32_t q_lo = ptx::smem_desc_lo(ptx::smem_u32(s.q)), k_lo = ptx::smem_desc_lo(ptx::smem_u32(s.k));
+    const uint32_t q_half16 = uint32_t(a.q_half_bytes) >> 4;
+    int ks = 0, kph = 0, as = 0, aph = 0, n_q = 0, trace_n = 0;
+    bool new_group = true;
+    int t = u0 % a.tpg;
+    TcCursor g; g.init(a, u0 / a.tpg);
+    for (int u = u0; u < u1; ++u) {
+      const int rs32 = (g.rs_valid(a) + 31) & ~31;
+      if (new_group) { ptx::mbar_wait(b.q_full, n_q & 1); ++n_q; new_group = false; }
+      ptx::mbar_wait(&b.k_full[ks], kph);
+      if (lane == 0) TC_TRACE(1, 1);
+      const uint32_t ka_lo = k_lo + uint32_t(ks) * (kTcKStage >> 4);
       for (int c0 = 0; c0 < rs32; c0 += 256) {                           // probe-row chunks of <= 256 columns
         const int nc = min(256, rs32 - c0);
-        ptx::mbar_wait(&t_empty[as], aph ^ 1);
+        ptx::mbar_wait(&b.t_empty[as], aph ^ 1);
         ptx::tc_fence_after();
-        if (lane == 0) {
-          const uint32_t idesc = ptx::idesc_bf16_f32(128, nc);
+        if (lane == 0) TC_TRACE(1, 2);
+        const uint32_t idesc = ptx::idesc_bf16_f32(128, nc);
+        const uint32_t qb_lo = q_lo + uint32_t(c0) * 8u;                 // c0 rows x 128 B >> 4
+        if (ptx::elect_one()) {
 #pragma unroll
-          for (int kk = 0; kk < 8; ++kk) {
-            const int h = kk >> 2;
-            const uint64_t ad = ptx::smem_desc_sw128(ptx::smem_u32(s.k + ks * KSTAGE + h * 16384)) + uint64_t((kk & 3) * 2);
-            const uint64_t bd = ptx::smem_desc_sw128(ptx::smem_u32(s.q + h * kTcQHalfBytes + c0 * 128)) + uint64_t((kk & 3) * 2);
-            ptx::mma_bf16(tmem_base + as * 256, ad, bd, idesc, kk > 0);
-          }
-          ptx::mma_commit(&t_full[as]);
+          for (int kk = 0; kk < 8; ++kk)
+            ptx::mma_bf16_lohi(tmem_base + as * 256, ka_lo + (kk >> 2) * 1024u + (kk & 3) * 2,
+                               qb_lo + (kk >> 2) * q_half16 + (kk & 3) * 2, ptx::kSmemDescHiSw128, idesc, kk > 0);
+          ptx::mma_commit(&b.t_full[as]);
         }
         __syncwarp();
+        if (lane == 0) TC_TRACE(1, 3);
         if (++as == 2) { as = 0; aph ^= 1; }
       }
-      if (lane == 0) {
-        ptx::mma_commit(&k_empty[ks]);
-        const bool last_of_group = (u + 1 == u1) || int((u + 1) / a.tpg) != gi;
-        if (last_of_group) ptx::mma_commit(q_empty);
+      const bool last_of_group = (u + 1 == u1) || t + 1 == a.tpg;
+      if (ptx::elect_one()) {
+        ptx::mma_commit(&b.k_empty[ks]);
+        if (last_of_group) ptx::mma_commit(b.q_empty);
       }
       __syncwarp();
-      if (++ks == NS) { ks = 0; kph ^= 1; }
+      if (++ks == a.n_kst) { ks = 0; kph ^= 1; }
+      if (++t == a.tpg) { t = 0; g.next(a); new_group = true; }
     }
   } else {
-    // ---------------- epilogue: one token per thread, two warps (column halves) per 32-lane quarter ----
-    const int e = warp - 2, half = e >> 2, lg = warp & 3;
+    // ---------------- epilogue: one token per thread; warp (lane quarter lg, column quarter cq) ----------------
+    const int e = warp - 2, cq = e >> 2, lg = warp & 3;
     const int tok_in_tile = lg * 32 + lane;
-    const int et = threadIdx.x - 64;                                     // 0..255
-    int as = 0, aph = 0, prev = -1, rs32 = 0;
-    TcGroup gr{};
-    for (long long u = u0; u < u1; ++u) {
-      const int gi = int(u / a.tpg), t = int(u % a.tpg);
-      if (gi != prev) {
-        gr = tc_group(a, gi); prev = gi;
-        rs32 = (gr.rs_valid + 31) & ~31;
-        ptx::named_bar_sync(1, 256);                                     // everyone is done with the old c_r
-        // merge the row's per-segment (m, z) of pass 1 in segment order: c_r = m_r + log2 Z_r
-        const float* pr = a.g.partial + (size_t(gr.bl) * a.g.Hq * a.g.p_max + gr.stat_row0) * a.spg * 2;
-        for (int i = et; i < kTcRowsMax; i += 256) {
-          float c = INFINITY;                                            // rows past the group: exp2(-inf) = 0
-          if (i < gr.rs_valid) {
-            const float2* p2 = reinterpret_cast<const float2*>(pr + size_t(i) * a.spg * 2);
-            float m = -INFINITY;
-            for (int j = 0; j < a.spg; ++j) m = fmaxf(m, p2[j].x);
-            float z = 0.f;
-            for (int j = 0; j < a.spg; ++j) z += p2[j].y * fast_exp2(p2[j].x - m);
-            c = m + log2f(z);
-          }
-          s.c[i] = c;
+    const uint32_t t_addr = tmem_base + (uint32_t(lg * 32) << 16) + cq * 32;
+    int as = 0, aph = 0, trace_n = 0;
+    const int trole = e == 0 ? 2 : 3;
+    const bool tr = kTrace && lane == 0 && (e == 0 || e == kTcEpiWarps - 1);
+    float v[32];
+    float acc[4] = {0.f, 0.f, 0.f, 0.f};
+    bool new_group = true;
+    int t = u0 % a.tpg, rs32 = 0;
+    float* col = nullptr;                                                // this warp's column-sum slot of the group
+    TcCursor g; g.init(a, u0 / a.tpg);
+    // sum over the 32 probe rows [col0, col0 + 32) of this token (32 registers live: no spills in this loop --
+    // a local-memory load would queue behind the exp2 traffic like every other MIO instruction)
+    auto fold = [&](int col0) {
+      const float4* c4 = reinterpret_cast<const float4*>(s.c + col0);
+      if (kVar & 1) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const float4 c = c4[j];
+          acc[0] += fast_exp2(fmaf(v[4 * j], a.scale_log2, -c.x));
+          acc[1] += fast_exp2(fmaf(v[4 * j + 1], a.scale_log2, -c.y));
+          acc[2] += fast_exp2(fmaf(v[4 * j + 2], a.scale_log2, -c.z));
+          acc[3] += fast_exp2(fmaf(v[4 * j + 3], a.scale_log2, -c.w));
         }
-        ptx::named_bar_sync(1, 256);
-      }
-      float acc[4] = {0.f, 0.f, 0.f, 0.f};
-      // 32 probe rows of this token: FFMA, MUFU and FADD phases kept apart so no warp waits on its own exp
-      auto fold = [&](float (&v)[32], int col) {
-        const float4* c4 = reinterpret_cast<const float4*>(s.c + col);
+      } else {
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
           const float4 c = c4[j];
@@ -398,47 +449,54 @@ k_tc_colsum(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ 
         for (int j = 0; j < 32; ++j) v[j] = fast_exp2(v[j]);
 #pragma unroll
         for (int j = 0; j < 32; j += 4) { acc[0] += v[j]; acc[1] += v[j + 1]; acc[2] += v[j + 2]; acc[3] += v[j + 3]; }
-      };
+      }
+    };
+    for (int u = u0; u < u1; ++u) {
+      if (new_group) {
+        ptx::named_bar_sync(1, kTcEpiWarps * 32);                        // everyone is done with the old c_r
+        if (tr) TC_TRACE(trole, 5);
+        const int bl = g.bl(a), rows_total = a.g.Hq * a.g.p_max;
+        tc_merge_rows(reinterpret_cast<const float2*>(a.g.partial) + size_t(bl) * (2 * a.spg) * rows_total + g.stat_row0(a),
+                      2 * a.spg, rows_total, g.rs_valid(a), s.c, threadIdx.x - 64);
+        ptx::named_bar_sync(1, kTcEpiWarps * 32);
+        if (tr) TC_TRACE(trole, 6);
+        rs32 = (g.rs_valid(a) + 31) & ~31;
+        col = a.g.colsum + (size_t(bl) * a.g.n_vh_max + (g.kvh * a.n_sc + g.sc) * 4 + cq) * a.g.cap;
+        new_group = false;
+      }
       for (int c0 = 0; c0 < rs32; c0 += 256) {
         const int nc = min(256, rs32 - c0);
-        ptx::mbar_wait(&t_full[as], aph);
+        const bool b0 = cq * 32 < nc, b1 = (cq + 4) * 32 < nc;           // this warp's 32-column blocks: cq and cq + 4
+        ptx::mbar_wait(&b.t_full[as], aph);
         ptx::tc_fence_after();
-        // this warp's 32-column blocks (every other one): the next block's TMEM load is in flight while
-        // the current one goes through the MUFU pipe
-        const uint32_t tbase = tmem_base + (uint32_t(lg * 32) << 16) + as * 256 + half * 32;
-        const int nb = (nc - half * 32 + 63) / 64;
-        float vA[32], vB[32];
-        if (nb > 0) ptx::tmem_ld32(tbase, vA);
-        for (int k = 0; k < nb; k += 2) {
+        if (tr) TC_TRACE(trole, 1);
+        if (b0) {
+          ptx::tmem_ld32(t_addr + as * 256, v);
           ptx::tmem_ld_wait();
-          if (k + 1 < nb) ptx::tmem_ld32(tbase + (k + 1) * 64, vB);
-          fold(vA, c0 + half * 32 + k * 64);
-          if (k + 1 < nb) {
-            ptx::tmem_ld_wait();
-            if (k + 2 < nb) ptx::tmem_ld32(tbase + (k + 2) * 64, vA);
-            fold(vB, c0 + half * 32 + (k + 1) * 64);
-          }
+          fold(c0 + cq * 32);
+        }
+        if (b1) {
+          ptx::tmem_ld32(t_addr + as * 256 + 128, v);
+          ptx::tmem_ld_wait();
         }
         ptx::tc_fence_before();
         __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(&t_empty[as]);
+        if (lane == 0) ptx::mbar_arrive(&b.t_empty[as]);                 // this warp's share of the stage is in registers
+        if (tr) TC_TRACE(trole, 2);
         if (++as == 2) { as = 0; aph ^= 1; }
+        if (b1) fold(c0 + (cq + 4) * 32);
+        if (tr) TC_TRACE(trole, 3);
       }
-      // merge the two column halves (one 64-thread barrier per lane quarter, double-buffered exchange)
-      // and store W's per-(KV head, super-chunk) column sum of this token
-      const float mine = (acc[0] + acc[1]) + (acc[2] + acc[3]);
-      const int par = int(u & 1);
-      if (half == 1) acc_x[par][tok_in_tile] = mine;
-      ptx::named_bar_sync(2 + lg, 64);
-      if (half == 0) {
-        const int tok = t * TN + tok_in_tile;
-        if (tok < a.Tn)
-          a.g.colsum[(size_t(gr.bl) * a.g.n_vh_max + gr.kvh * a.n_sc + gr.sc) * a.g.cap + tok] = mine + acc_x[par][tok_in_tile];
-      }
+      // per-(KV head, super-chunk, column quarter) column sum of this token; k_wsum adds the slots in order
+      const int tok = t * kTcTile + tok_in_tile;
+      if (tok < a.Tn) col[tok] = (acc[0] + acc[1]) + (acc[2] + acc[3]);
+      acc[0] = acc[1] = acc[2] = acc[3] = 0.f;
+      if (++t == a.tpg) { t = 0; g.next(a); new_group = true; }
     }
   }
   ptx::tc_fence_before();
   __syncthreads();
+  if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.trace[4 * kTcTraceN + 2 * blockIdx.x + 1] = t; }
   if (warp == 1) ptx::tmem_dealloc(tmem_base, 512);
 }
 
@@ -457,6 +515,11 @@ struct TcState {
   EncodeTiledFn encode = nullptr;
   CUtensorMap tmap_k;
   int n_sm = 0;
+  long long* trace = nullptr;   // 2 kernels x 4 roles x kTcTraceN events (HERMES_TC_TRACE=<file>)
+  std::string trace_path;
+  void (*k_stats)(CUtensorMap, CUtensorMap, TcArgs) = nullptr;
+  void (*k_colsum)(CUtensorMap, CUtensorMap, TcArgs) = nullptr;
+  int var1 = 0, var2 = 0;   // experiment switches (HERMES_TC_VAR1 / HERMES_TC_VAR2)
 };
 
 // 2D bf16 tensor map over [rows][cols] (cols contiguous), 64 x 64 boxes, 128-byte swizzle, zero OOB fill.
@@ -487,12 +550,20 @@ inline bool tc_init(hermes_t* h) {
   cudaDeviceProp prop;
   if (cudaGetDeviceProperties(&prop, c.device) != cudaSuccess) { h->err = "cudaGetDeviceProperties failed"; delete st; return false; }
   st->n_sm = prop.multiProcessorCount;
+  if (const char* e = getenv("HERMES_TC_TRACE")) {
+    st->trace_path = e;
+    if (cudaMalloc(&st->trace, 2 * kTcTraceStride * 8) != cudaSuccess) st->trace = nullptr;
+  }
+  if (const char* e = getenv("HERMES_TC_VAR1")) st->var1 = atoi(e);
+  if (const char* e = getenv("HERMES_TC_VAR2")) st->var2 = atoi(e);
   const Geom& g = h->geom;
   if (!tc_make_map(st, &st->tmap_k, g.kc, uint64_t(g.row_elems), uint64_t(g.B) * g.L * 2 * g.cap)) {
     h->err = "cuTensorMapEncodeTiled(K cache) failed"; delete st; return false;
   }
-  if (cudaFuncSetAttribute(k_tc_stats, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) != cudaSuccess ||
-      cudaFuncSetAttribute(k_tc_colsum, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes) != cudaSuccess) {
+  st->k_stats = st->trace ? k_tc_stats<0, true> : (st->var1 & 1) ? k_tc_stats<1, false> : k_tc_stats<0, false>;
+  st->k_colsum = st->trace ? k_tc_colsum<0, true> : (st->var2 & 1) ? k_tc_colsum<1, false> : k_tc_colsum<0, false>;
+  if (cudaFuncSetAttribute(st->k_stats, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemMax) != cudaSuccess ||
+      cudaFuncSetAttribute(st->k_colsum, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemMax) != cudaSuccess) {
     h->err = std::string("cudaFuncSetAttribute(tc kernels): ") + cudaGetErrorString(cudaGetLastError());
     delete st; return false;
   }
@@ -501,7 +572,15 @@ inline bool tc_init(hermes_t* h) {
 }
 
 inline void tc_destroy(hermes_t* h) {
-  delete static_cast<TcState*>(h->tc_state);
+  TcState* st = static_cast<TcState*>(h->tc_state);
+  if (st && st->trace) {                         // diagnostics: dump the last update's event trace
+    std::vector<long long> host(2 * kTcTraceStride);
+    cudaDeviceSynchronize();
+    if (cudaMemcpy(host.data(), st->trace, host.size() * 8, cudaMemcpyDeviceToHost) == cudaSuccess)
+      if (FILE* f = fopen(st->trace_path.c_str(), "wb")) { fwrite(host.data(), 8, host.size(), f); fclose(f); }
+    cudaFree(st->trace);
+  }
+  delete st;
   h->tc_state = nullptr;
 }
 
@@ -534,21 +613,26 @@ inline int tc_score(hermes_t* h, const void* q_probe, int Tn, int P, float scale
   a.RS = ((a.R + a.n_sc - 1) / a.n_sc + 31) & ~31;            // rows per super-chunk, multiple of 32
   a.n_sc = (a.R + a.RS - 1) / a.RS;
   a.n_groups = g.B * (g.L - g.n_shallow) * g.Hkv * a.n_sc;
-  const int tpg1 = (Tn + 63) / 64, tpg2 = (Tn + 127) / 128;
-  a.spg = (tpg1 + kTcSegTiles - 1) / kTcSegTiles;
-  const long long U1 = (long long)a.n_groups * a.spg, U2 = (long long)a.n_groups * tpg2;
+  a.tpg = (Tn + kTcTile - 1) / kTcTile;
+  a.spg = (a.tpg + kTcSegTiles - 1) / kTcSegTiles;
+  const long long U1 = (long long)a.n_groups * a.spg, U2 = (long long)a.n_groups * a.tpg;
+  if (U2 > INT_MAX / 2) { h->err = "tcgen05 scoring: too many (group, tile) units"; return HERMES_ECAPACITY; }
   const int n_cta1 = int(std::min<long long>(st->n_sm, U1)), n_cta2 = int(std::min<long long>(st->n_sm, U2));
-  if (a.spg > h->lay.n_part_max || g.Hkv * a.n_sc > g.n_vh_max) { h->err = "internal: tc scratch too small"; return HERMES_ESTATE; }
-  h->n_vh = g.Hkv * a.n_sc;
+  if (2 * a.spg > h->lay.n_part_max || g.Hkv * a.n_sc * 4 > g.n_vh_max) { h->err = "internal: tc scratch too small"; return HERMES_ESTATE; }
+  h->n_vh = g.Hkv * a.n_sc * 4;
+  a.q_half_bytes = (a.RS + 63) / 64 * 8192;
+  a.n_kst = std::min(kTcKStagesMax, (kTcSmemMax - tc_smem_bytes(a.q_half_bytes, 0)) / kTcKStage);
+  const int smem = tc_smem_bytes(a.q_half_bytes, a.n_kst);
   {
     TcProf p(h, HERMES_K_SCORE_STATS, s);
-    a.tpg = tpg1;
-    k_tc_stats<<<n_cta1, kTcStatsThreads, kTcSmemBytes, s>>>(tmap_q, st->tmap_k, a);
+    a.trace = st->trace;
+    if (st->trace) cudaMemsetAsync(st->trace, 0, 2 * kTcTraceStride * 8, s);
+    st->k_stats<<<n_cta1, kTcThreads, smem, s>>>(tmap_q, st->tmap_k, a);
   }
   {
     TcProf p(h, HERMES_K_SCORE_COLSUM, s);
-    a.tpg = tpg2;
-    k_tc_colsum<<<n_cta2, kTcColsumThreads, kTcSmemBytes, s>>>(tmap_q, st->tmap_k, a);
+    a.trace = st->trace ? st->trace + kTcTraceStride : nullptr;
+    st->k_colsum<<<n_cta2, kTcThreads, smem, s>>>(tmap_q, st->tmap_k, a);
   }
   return HERMES_OK;
 }
