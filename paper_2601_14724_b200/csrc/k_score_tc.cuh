@@ -258,7 +258,7 @@ k_tc_stats(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ C
 #pragma unroll
         for (int j = 0; j < 64; j += 4) {
 #pragma unroll
-          for (int i = 0; i < 4; ++i) sm[i] += fast_exp2(fmaf(v[j + i], a.scale_log2, -m_new));
+          for (int i = 0; i < 4; ++i) sm[i] += exp2_mix<(kVar >> 1)>(fmaf(v[j + i], a.scale_log2, -m_new), j + i);
         }
       } else {                                                           // three phases
 #pragma unroll
@@ -431,10 +431,10 @@ k_tc_colsum(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ 
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
           const float4 c = c4[j];
-          acc[0] += fast_exp2(fmaf(v[4 * j], a.scale_log2, -c.x));
-          acc[1] += fast_exp2(fmaf(v[4 * j + 1], a.scale_log2, -c.y));
-          acc[2] += fast_exp2(fmaf(v[4 * j + 2], a.scale_log2, -c.z));
-          acc[3] += fast_exp2(fmaf(v[4 * j + 3], a.scale_log2, -c.w));
+          acc[0] += exp2_mix<(kVar >> 1)>(fmaf(v[4 * j], a.scale_log2, -c.x), 4 * j);
+          acc[1] += exp2_mix<(kVar >> 1)>(fmaf(v[4 * j + 1], a.scale_log2, -c.y), 4 * j + 1);
+          acc[2] += exp2_mix<(kVar >> 1)>(fmaf(v[4 * j + 2], a.scale_log2, -c.z), 4 * j + 2);
+          acc[3] += exp2_mix<(kVar >> 1)>(fmaf(v[4 * j + 3], a.scale_log2, -c.w), 4 * j + 3);
         }
       } else {
 #pragma unroll
@@ -560,8 +560,16 @@ inline bool tc_init(hermes_t* h) {
   if (!tc_make_map(st, &st->tmap_k, g.kc, uint64_t(g.row_elems), uint64_t(g.B) * g.L * 2 * g.cap)) {
     h->err = "cuTensorMapEncodeTiled(K cache) failed"; delete st; return false;
   }
-  st->k_stats = st->trace ? k_tc_stats<0, true> : (st->var1 & 1) ? k_tc_stats<1, false> : k_tc_stats<0, false>;
-  st->k_colsum = st->trace ? k_tc_colsum<0, true> : (st->var2 & 1) ? k_tc_colsum<1, false> : k_tc_colsum<0, false>;
+  auto pick1 = [](int v) -> void (*)(CUtensorMap, CUtensorMap, TcArgs) {
+    switch (v) { case 1: return k_tc_stats<1, false>; case 3: return k_tc_stats<3, false>; case 5: return k_tc_stats<5, false>;
+                 case 7: return k_tc_stats<7, false>; case 9: return k_tc_stats<9, false>; default: return k_tc_stats<0, false>; }
+  };
+  auto pick2 = [](int v) -> void (*)(CUtensorMap, CUtensorMap, TcArgs) {
+    switch (v) { case 1: return k_tc_colsum<1, false>; case 3: return k_tc_colsum<3, false>; case 5: return k_tc_colsum<5, false>;
+                 case 7: return k_tc_colsum<7, false>; case 9: return k_tc_colsum<9, false>; default: return k_tc_colsum<0, false>; }
+  };
+  st->k_stats = st->trace ? k_tc_stats<0, true> : pick1(st->var1);
+  st->k_colsum = st->trace ? k_tc_colsum<0, true> : pick2(st->var2);
   if (cudaFuncSetAttribute(st->k_stats, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemMax) != cudaSuccess ||
       cudaFuncSetAttribute(st->k_colsum, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemMax) != cudaSuccess) {
     h->err = std::string("cudaFuncSetAttribute(tc kernels): ") + cudaGetErrorString(cudaGetLastError());
