@@ -26,6 +26,10 @@ from workloads import CONFIGS, chunk_kv, probe_q  # noqa: E402
 
 METRIC, UNIT = "kv_tokens_managed_per_s", "tokens/s"
 POOL = 16          # distinct pre-generated chunk/probe sets cycled through the timed region
+# dram__bytes_read.sum + dram__bytes_write.sum per launch at configs[1], transcribed from the one
+# `ncu --set full` capture summarised in profiles/r1b_ncu_full_summary.txt (command in profiles/r1b_README.md)
+NCU_TRAFFIC_BYTES = {"gather": 361.28e6 + 311.93e6, "score_stats": 184.26e6 + 7.40e6, "score_colsum": 200.97e6 + 9.88e6,
+                     "select": 1.44e6, "append": 11.25e6}
 
 
 # ------------------------------------------------------------------------------- shared helpers
@@ -206,10 +210,7 @@ def run_ours(args):
     kern = {k: v for k, v in acc.items() if v > 0}
     dom = max(kern, key=kern.get)
     t_dom = kern[dom] * 1e-3
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tp):
-        traffic = json.load(open(tp)).get(dom)
+    traffic = NCU_TRAFFIC_BYTES.get(dom) if args.workload == "llava_ov_7b" else None
     if dom == "gather" or dom == "append":
         ach = work["gather_bytes"] / t_dom / 1e9
         roof = dict(kernel=dom, bound="hbm", achieved=ach, peak=pk["hbm"], unit="GB/s", frac=ach / pk["hbm"], traffic=traffic)
