@@ -121,6 +121,13 @@ __device__ __forceinline__ float exp2_mix(float x, int j) {
   return ((j & 7) * kPoly) % 8 < kPoly && kPoly > 0 ? exp2_poly(x) : fast_exp2(x);
 }
 
+// Programmatic dependent launch: every kernel of an update is launched with the programmatic-stream-
+// serialization attribute, so its CTAs may become resident (and run their prologue) while the previous
+// kernel drains.  pdl_wait() blocks until the previous kernel has completed and its writes are visible;
+// data written by earlier kernels is then read with ld.global.cg (L2), never through a possibly stale L1 line.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 __device__ inline float warp_max(float v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));

@@ -274,8 +274,8 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
     Prof p(h, HERMES_K_APPEND, s);
     const size_t n_vec = size_t(n_new) * row_vecs;
     const int gx = int(std::min<size_t>((n_vec + 511) / 512, 64));
-    k_append<<<dim3(std::max(gx, 1), BL), 256, 0, s>>>(g, static_cast<const uint4*>(K_new), static_cast<const uint4*>(V_new),
-                                                      h->cur, h->len, n_new, row_vecs, int(p0));
+    launch_pdl(k_append, dim3(std::max(gx, 1), BL), dim3(256), 0, s, g, static_cast<const uint4*>(K_new), static_cast<const uint4*>(V_new),
+               h->cur, h->len, n_new, row_vecs, int(p0));
   }
   if (evict) {
     const float scale = c.softmax_scale > 0.f ? c.softmax_scale : float(1.0 / std::sqrt(double(c.head_dim)));
@@ -299,8 +299,8 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
       const double k = c.forget_rate;
       const float r_norm_sum = float((1.0 - std::exp(-k)) / (1.0 - std::exp(-k * Tn)));
       if (g.L > g.n_shallow)
-        k_wsum<<<dim3((Tn + 255) / 256, g.B * (g.L - g.n_shallow)), 256, 0, s>>>(g, Tn, n_probe, h->n_vh);
-      k_select<<<BL, kSelThreads, size_t(Tn) * 4, s>>>(g, h->cur, Tn, c.forget_rate, c.norm_mode == HERMES_NORM_SUM, r_norm_sum);
+        launch_pdl(k_wsum, dim3((Tn + 255) / 256, g.B * (g.L - g.n_shallow)), dim3(256), 0, s, g, Tn, n_probe, h->n_vh);
+      launch_pdl(k_select, dim3(BL), dim3(kSelThreads), size_t(Tn) * 4, s, g, h->cur, Tn, c.forget_rate, int(c.norm_mode == HERMES_NORM_SUM), r_norm_sum);
     }
     {
       Prof p(h, HERMES_K_GATHER, s);
@@ -312,11 +312,11 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
       const int gx = std::max(1, std::min(want, (total + kGatherThreads - 1) / kGatherThreads));
       const dim3 grid(gx, BL);
       if (c.dtype == HERMES_BF16) {
-        if (g.n_axes == 1) k_gather<__nv_bfloat16, 1><<<grid, kGatherThreads, 0, s>>>(g, h->cur);
-        else k_gather<__nv_bfloat16, 3><<<grid, kGatherThreads, 0, s>>>(g, h->cur);
+        if (g.n_axes == 1) launch_pdl(k_gather<__nv_bfloat16, 1>, grid, dim3(kGatherThreads), 0, s, g, h->cur);
+        else launch_pdl(k_gather<__nv_bfloat16, 3>, grid, dim3(kGatherThreads), 0, s, g, h->cur);
       } else {
-        if (g.n_axes == 1) k_gather<float, 1><<<grid, kGatherThreads, 0, s>>>(g, h->cur);
-        else k_gather<float, 3><<<grid, kGatherThreads, 0, s>>>(g, h->cur);
+        if (g.n_axes == 1) launch_pdl(k_gather<float, 1>, grid, dim3(kGatherThreads), 0, s, g, h->cur);
+        else launch_pdl(k_gather<float, 3>, grid, dim3(kGatherThreads), 0, s, g, h->cur);
       }
     }
   }

@@ -106,6 +106,18 @@ inline Layout make_layout(const hermes_config& c) {
   return y;
 }
 
+// Launch with programmatic stream serialization allowed (see pdl_wait() in common.cuh).
+template <typename... P, typename... A>
+inline cudaError_t launch_pdl(void (*kernel)(P...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, A... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, P(args)...);
+}
+
 struct KernelTimer {
   cudaEvent_t beg[HERMES_K_COUNT]{}, end[HERMES_K_COUNT]{};
   bool ran[HERMES_K_COUNT]{};

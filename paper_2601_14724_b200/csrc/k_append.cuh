@@ -10,6 +10,8 @@ namespace hk {
 __global__ void __launch_bounds__(256)
 k_append(Geom g, const uint4* __restrict__ k_new, const uint4* __restrict__ v_new,
          int cur, int len, int n_new, int row_vecs, int pos_start) {
+  pdl_wait();
+  pdl_launch_dependents();
   const int bl = blockIdx.y;                        // b * L + l
   if (blockIdx.x == 0 && threadIdx.x == 0) g.wmax[bl] = 0u;   // reset the per-layer max of W for this step
   const size_t slab = size_t(bl) * 2 + cur;

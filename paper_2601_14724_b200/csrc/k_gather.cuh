@@ -76,6 +76,8 @@ __device__ __forceinline__ void rotate_unit(const Geom& g, const int (&dl)[NAX],
 template <typename T, int NAX>
 __global__ void __launch_bounds__(kGatherThreads, 4)
 k_gather(Geom g, int cur) {
+  pdl_wait();
+  pdl_launch_dependents();
   constexpr int V = Elem<T>::kPerVec;
   const int bl = blockIdx.y;
   const int half = g.d >> 1;
@@ -94,10 +96,10 @@ k_gather(Geom g, int cur) {
   int idx = blockIdx.x * kGatherThreads + threadIdx.x;
   if (idx >= total) return;
   int s = idx / upr;
-  int src = __ldg(kept + s);
+  int src = __ldcg(kept + s);
   int dl[NAX];
 #pragma unroll
-  for (int a = 0; a < NAX; ++a) dl[a] = __ldg(delta + a * g.budget + s);
+  for (int a = 0; a < NAX; ++a) dl[a] = __ldcg(delta + a * g.budget + s);
 
 #pragma unroll 1
   while (true) {
@@ -110,10 +112,10 @@ k_gather(Geom g, int cur) {
     const int idx_n = idx + stride;
     const bool more = idx_n < total;
     const int s_n = more ? idx_n / upr : s;
-    const int src_n = __ldg(kept + s_n);
+    const int src_n = __ldcg(kept + s_n);
     int dl_n[NAX];
 #pragma unroll
-    for (int a = 0; a < NAX; ++a) dl_n[a] = __ldg(delta + a * g.budget + s_n);
+    for (int a = 0; a < NAX; ++a) dl_n[a] = __ldcg(delta + a * g.budget + s_n);
 
     bool any = false;
 #pragma unroll

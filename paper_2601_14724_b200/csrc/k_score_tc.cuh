@@ -178,6 +178,8 @@ k_tc_stats(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ C
   const int s0 = tc_unit_begin(U, gridDim.x, blockIdx.x), s1 = tc_unit_begin(U, gridDim.x, blockIdx.x + 1);
   if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.trace[4 * kTcTraceN + 2 * blockIdx.x] = t; }
   const uint32_t tmem_base = tc_prologue(s, b, a, &tmap_q, &tmap_k);
+  pdl_wait();                       // the chunk's K rows come from k_append
+  if (threadIdx.x == 0) pdl_launch_dependents();
 
   if (warp == 0) {
     if (lane == 0) tc_producer<true, kTrace>(s, b, &tmap_q, &tmap_k, a, s0, s1);
@@ -331,7 +333,7 @@ __device__ __noinline__ void tc_merge_rows(const float2* pr, int n_slot, int row
       for (int j0 = 0; j0 < n_slot; j0 += 16) {
         float2 pv[16];
 #pragma unroll
-        for (int j = 0; j < 16; ++j) pv[j] = __ldg(p2 + size_t(min(j0 + j, n_slot - 1)) * rows_total);   // always in range: no branch
+        for (int j = 0; j < 16; ++j) pv[j] = __ldcg(p2 + size_t(min(j0 + j, n_slot - 1)) * rows_total);   // always in range: no branch
 #pragma unroll
         for (int j = 0; j < 16; ++j) if (j0 + j >= n_slot) pv[j] = make_float2(-INFINITY, 0.f);
         float mc = m;
@@ -365,6 +367,8 @@ k_tc_colsum(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ 
   const int u0 = tc_unit_begin(U, gridDim.x, blockIdx.x), u1 = tc_unit_begin(U, gridDim.x, blockIdx.x + 1);
   if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.trace[4 * kTcTraceN + 2 * blockIdx.x] = t; }
   const uint32_t tmem_base = tc_prologue(s, b, a, &tmap_q, &tmap_k);
+  if (threadIdx.x == 0) pdl_launch_dependents();
+  // producer and MMA warps start at once (K and Q do not depend on pass 1); the epilogue waits for pass 1
 
   if (warp == 0) {
     if (lane == 0) tc_producer<false, kTrace>(s, b, &tmap_q, &tmap_k, a, u0, u1);
@@ -411,6 +415,7 @@ k_tc_colsum(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ 
     }
   } else {
     // ---------------- epilogue: one token per thread; warp (lane quarter lg, column quarter cq) ----------------
+    pdl_wait();
     const int e = warp - 2, cq = e >> 2, lg = warp & 3;
     const int tok_in_tile = lg * 32 + lane;
     const uint32_t t_addr = tmem_base + (uint32_t(lg * 32) << 16) + cq * 32;
@@ -635,12 +640,12 @@ inline int tc_score(hermes_t* h, const void* q_probe, int Tn, int P, float scale
     TcProf p(h, HERMES_K_SCORE_STATS, s);
     a.trace = st->trace;
     if (st->trace) cudaMemsetAsync(st->trace, 0, 2 * kTcTraceStride * 8, s);
-    st->k_stats<<<n_cta1, kTcThreads, smem, s>>>(tmap_q, st->tmap_k, a);
+    launch_pdl(st->k_stats, dim3(n_cta1), dim3(kTcThreads), size_t(smem), s, tmap_q, st->tmap_k, a);
   }
   {
     TcProf p(h, HERMES_K_SCORE_COLSUM, s);
     a.trace = st->trace ? st->trace + kTcTraceStride : nullptr;
-    st->k_colsum<<<n_cta2, kTcThreads, smem, s>>>(tmap_q, st->tmap_k, a);
+    launch_pdl(st->k_colsum, dim3(n_cta2), dim3(kTcThreads), size_t(smem), s, tmap_q, st->tmap_k, a);
   }
   return HERMES_OK;
 }

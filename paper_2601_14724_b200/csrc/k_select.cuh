@@ -84,13 +84,15 @@ __device__ inline int block_reduce_min_i(int v, int* scratch) {
 __global__ void __launch_bounds__(256)
 k_wsum(Geom g, int Tn, int P, int n_vh) {
   __shared__ float red[8];
+  pdl_wait();
+  pdl_launch_dependents();
   const int Ls = g.L - g.n_shallow;
   const int bl = (blockIdx.y / Ls) * g.L + g.n_shallow + blockIdx.y % Ls;
   const int i = blockIdx.x * 256 + threadIdx.x;
   float w = 0.f;
   if (i < Tn) {
     const float* c = g.colsum + size_t(bl) * g.n_vh_max * g.cap + i;
-    for (int h = 0; h < n_vh; ++h) w += c[size_t(h) * g.cap];
+    for (int h = 0; h < n_vh; ++h) w += __ldcg(c + size_t(h) * g.cap);
     w *= 1.0f / float(g.Hq * P);
     g.wsum[size_t(bl) * g.cap + i] = w;
   }
@@ -121,6 +123,8 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
 #ifdef HERMES_SELECT_TIMING
   __shared__ long long tstamp[8];
 #endif
+  pdl_wait();
+  pdl_launch_dependents();
   SEL_T(0);
   const int bl = blockIdx.x, l = bl % g.L;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -134,12 +138,12 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
   float n0, n1;
   if (norm_sum) {
     float t0 = 0.f, t1 = 0.f;
-    for (int i = tid; i < Tn; i += kSelThreads) { if (scored0) t0 += w0[i]; if (scored1) t1 += w1[i]; }
+    for (int i = tid; i < Tn; i += kSelThreads) { if (scored0) t0 += __ldcg(w0 + i); if (scored1) t1 += __ldcg(w1 + i); }
     n0 = block_reduce_sum(t0, red_f);
     n1 = block_reduce_sum(t1, red_f);
   } else {
-    n0 = scored0 ? __uint_as_float(g.wmax[bl]) : 1.f;
-    n1 = scored1 ? __uint_as_float(g.wmax[bl + 1]) : 1.f;
+    n0 = scored0 ? __uint_as_float(__ldcg(g.wmax + bl)) : 1.f;
+    n1 = scored1 ? __uint_as_float(__ldcg(g.wmax + bl + 1)) : 1.f;
   }
   const float a0 = scored0 ? 1.0f / n0 : 0.f, a1 = scored1 ? 1.0f / n1 : 0.f;
   const float om0 = g.omega[l], om1 = has_next ? g.omega[l + 1] : 0.f;
@@ -154,8 +158,8 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
       const int i = i0 + j * kSelThreads;
-      x0[j] = (scored0 && i < Tn) ? w0[i] : 0.f;
-      x1[j] = (scored1 && i < Tn) ? w1[i] : 0.f;
+      x0[j] = (scored0 && i < Tn) ? __ldcg(w0 + i) : 0.f;
+      x1[j] = (scored1 && i < Tn) ? __ldcg(w1 + i) : 0.f;
     }
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
@@ -271,7 +275,7 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
 #pragma unroll
     for (int j = 0; j < 8; ++j) {
       const int i = (cb + 32 * j) * 32 + lane;
-      p_old[j] = (g.n_axes == 1 && i < Tn) ? pos_old[i] : 0;
+      p_old[j] = (g.n_axes == 1 && i < Tn) ? __ldcg(pos_old + i) : 0;
     }
 #pragma unroll
     for (int j = 0; j < 8; ++j) {
@@ -308,26 +312,26 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
     int32_t* pn = pos_new + size_t(a) * g.cap;
     int32_t* dl = g.delta + (size_t(bl) * 3 + a) * g.budget;
     if (!((g.compact_axes >> a) & 1)) {                 // axis kept as is (DESIGN c13)
-      for (int s = tid; s < g.budget; s += kSelThreads) { pn[s] = po[kept[s]]; dl[s] = 0; }
+      for (int s = tid; s < g.budget; s += kSelThreads) { pn[s] = __ldcg(po + kept[s]); dl[s] = 0; }
       continue;
     }
     int vmin = INT_MAX, vmax_neg = INT_MAX;
     for (int s = tid; s < g.budget; s += kSelThreads) {
-      const int v = po[kept[s]];
+      const int v = __ldcg(po + kept[s]);
       vmin = min(vmin, v); vmax_neg = min(vmax_neg, -v);
     }
     vmin = block_reduce_min_i(vmin, red_i);
     const int vmax = -block_reduce_min_i(vmax_neg, red_i);
     if (vmax - vmin >= kBitmapWords * 32) {             // cannot rank: report, leave the axis untouched
       if (tid == 0) atomicOr(g.status, 1);
-      for (int s = tid; s < g.budget; s += kSelThreads) { pn[s] = po[kept[s]]; dl[s] = 0; }
+      for (int s = tid; s < g.budget; s += kSelThreads) { pn[s] = __ldcg(po + kept[s]); dl[s] = 0; }
       continue;
     }
     __syncthreads();
     for (int w = tid; w < kBitmapWords; w += kSelThreads) bitmap[w] = 0u;
     __syncthreads();
     for (int s = tid; s < g.budget; s += kSelThreads) {
-      const int v = po[kept[s]] - vmin;
+      const int v = __ldcg(po + kept[s]) - vmin;
       atomicOr(&bitmap[v >> 5], 1u << (v & 31));
     }
     __syncthreads();
@@ -338,7 +342,7 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
     word_prefix[2 * tid + 1] = wpre + __popc(bitmap[2 * tid]);
     __syncthreads();
     for (int s = tid; s < g.budget; s += kSelThreads) {
-      const int v = po[kept[s]] - vmin;
+      const int v = __ldcg(po + kept[s]) - vmin;
       const int p_new = g.pos_offset + word_prefix[v >> 5] + __popc(bitmap[v >> 5] & ((1u << (v & 31)) - 1u));
       pn[s] = p_new;
       dl[s] = p_new - (v + vmin);
