@@ -134,6 +134,7 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   up(g.omega, omega.data(), L * 4); up(g.lambda, lambda.data(), L * 4);
   up(g.rope_freq, freq.data(), half * 8); up(g.rope_tab, tab.data(), tab.size() * 8);
   if (e == cudaSuccess) e = cudaMemset(g.status, 0, 256);
+  if (e == cudaSuccess) e = cudaMemset(h->ws + y.seg_cnt, 0, size_t(g.B) * L * y.n_vh_max * 4);
   if (e == cudaSuccess) e = cudaMemset(g.posc, 0, size_t(g.B) * L * 2 * y.n_axes * y.cap * 4);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_select, cudaFuncAttributeMaxDynamicSharedMemorySize, y.cap * 4);
   if (e == cudaSuccess) e = cudaDeviceSynchronize();

@@ -16,7 +16,7 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {           // byte offsets into the workspace
   size_t kc, vc, posc, colsum, wsum, wmax, rowstat, partial, scores, kept, delta, rope_tab, rope_freq, omega, lambda,
-      status, stage_k, stage_v, stage_q, tmaps, total;
+      status, seg_cnt, stage_k, stage_v, stage_q, tmaps, total;
   int cap, n_axes, n_part_max, table_rows, n_shallow, n_middle, n_deep, n_vh_max;
   size_t esize, row_bytes;
 };
@@ -98,6 +98,7 @@ inline Layout make_layout(const hermes_config& c) {
   y.omega = take(size_t(c.n_layers) * 4);
   y.lambda = take(size_t(c.n_layers) * 4);
   y.status = take(256);
+  y.seg_cnt = take(BL * y.n_vh_max * 4);
   y.stage_k = take(BL * c.max_chunk_tokens * y.row_bytes);
   y.stage_v = take(BL * c.max_chunk_tokens * y.row_bytes);
   y.stage_q = take(BL * rows * c.head_dim * y.esize);

@@ -1,10 +1,10 @@
 // a1 -- attention importance W (Eq. 2) on the 5th-gen tensor cores: bf16, head_dim 128.
 //
-// Same two-pass recompute as the CUDA-core path (k_score_simt.cuh), but each pass is a persistent,
-// warp-specialised tcgen05 kernel fed by TMA, with fp32 accumulators in TMEM:
-//   pass 1 k_tc_stats  : D[row, tok] = Q_blk K_tile^T, probe rows on TMEM lanes -> each thread owns one
+// Same two-pass recompute as the CUDA-core path (k_score_simt.cuh), as ONE persistent, warp-specialised
+// tcgen05 kernel (k_tc_score) fed by TMA, with fp32 accumulators in TMEM:
+//   pass 1 (tc_pass1)  : D[row, tok] = Q_blk K_tile^T, probe rows on TMEM lanes -> each thread owns one
 //                        probe row and keeps its running (max, sum exp2) over the tokens: no cross-lane work.
-//   pass 2 k_tc_colsum : D[tok, row] = K_tile Q^T, tokens on TMEM lanes -> each thread owns one token and
+//   pass 2 (tc_pass2)  : D[tok, row] = K_tile Q^T, tokens on TMEM lanes -> each thread owns one token and
 //                        accumulates sum_r exp2(s * scale - c_r), c_r = m_r + log2 Z_r merged from pass 1.
 // A "group" = (stream, scored layer, KV head, row super-chunk of <= 512 probe rows); its Q rows stay in
 // shared memory while the 128-token K tiles of the group stream through a TMA ring.  The flattened
@@ -38,9 +38,11 @@ struct TcArgs {
   int R, RS, n_sc;          // probe rows per KV head (G*P), rows per super-chunk, super-chunks per KV head
   int tpg;                  // 128-token tiles per group
   int n_groups;             // B * Ls * Hkv * n_sc
-  int spg;                  // pass 1: 512-token segments per group; partial (m, z) slots per probe row = 2 * spg
+  int spg;                  // pass 1: 512-token segments per group = partial (m, z) slots per probe row
   int q_half_bytes;         // shared-memory bytes of one 64-column half of the group's Q rows (64-row boxes)
   int n_kst;                // K ring stages
+  unsigned* seg_cnt;        // [n_groups] pass-1 progress: += 16 (epilogue warps) per finished segment, never reset
+  unsigned seg_target;      // value of seg_cnt[g] once all pass-1 segments of THIS update are done
   long long* trace;         // optional event trace of CTA 0 (HERMES_TC_TRACE; NULL in production)
 };
 
@@ -49,8 +51,8 @@ constexpr int kTcTraceN = 1024;
 constexpr int kTcTraceStride = 4 * kTcTraceN + 512;   // per kernel: 4 roles of CTA 0 + (start, end) globaltimer of every CTA
 #define TC_TRACE(role, id)                                                              \
   do {                                                                                  \
-    if (kTrace && a.trace != nullptr && blockIdx.x == 0 && trace_n < kTcTraceN)         \
-      a.trace[(role) * kTcTraceN + trace_n++] = (clock64() << 4) | (id);                \
+    if (kTrace && trace_p != nullptr && blockIdx.x == 0 && trace_n < kTcTraceN)         \
+      trace_p[(role) * kTcTraceN + trace_n++] = (clock64() << 4) | (id);                \
   } while (0)
 
 // ---- schedule: CTA c owns flattened units [c*U/nC, (c+1)*U/nC) -----------------------------------
@@ -78,11 +80,12 @@ struct TcSmem {
   uint8_t* q;        // [2 halves][q_half_bytes / 128 rows][128 B], 128B-swizzled
   uint8_t* k;        // K ring: [stage][2 halves][128 tokens][128 B]
   float* c;          // [512] per-row c_r (pass 2)
+  float4* xch;       // [2][8][32] pass-1 exchange between the two token-half warps of a row block quarter
   uint64_t* bars;    // mbarriers
   uint32_t* tmem;    // TMEM base address written by tcgen05.alloc
 };
 __host__ __device__ inline int tc_smem_bytes(int q_half_bytes, int n_kst) {
-  return 1024 + 2 * q_half_bytes + n_kst * kTcKStage + kTcRowsMax * 4 + 256 + 16;
+  return 1024 + 2 * q_half_bytes + n_kst * kTcKStage + kTcRowsMax * 4 + 8192 + 256 + 16;
 }
 __device__ inline TcSmem tc_carve(uint8_t* raw, const TcArgs& a) {
   uint8_t* p = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(raw) + 1023) & ~uintptr_t(1023));
@@ -90,6 +93,7 @@ __device__ inline TcSmem tc_carve(uint8_t* raw, const TcArgs& a) {
   s.q = p; p += 2 * a.q_half_bytes;
   s.k = p; p += a.n_kst * kTcKStage;
   s.c = reinterpret_cast<float*>(p); p += kTcRowsMax * 4;
+  s.xch = reinterpret_cast<float4*>(p); p += 8192;
   s.bars = reinterpret_cast<uint64_t*>(p); p += 256;
   s.tmem = reinterpret_cast<uint32_t*>(p);
   return s;
@@ -121,15 +125,19 @@ __device__ inline uint32_t tc_prologue(const TcSmem& s, const TcBars& b, const T
   return *s.tmem;
 }
 
+// Pipeline state a thread carries from pass 1 into pass 2 (ring slot / phase of the K ring, TMEM stage /
+// phase, number of Q loads so far); which fields a thread uses depends on its role.
+struct TcRole { int ks = 0, kph = 0, as = 0, aph = 0, n_q = 0; };
+
 // TMA producer (one thread), identical for both passes: the 128-token K tiles of units [u0, u1) and the
 // Q rows of each group the CTA touches (both 64-column halves, 64-row boxes).  kSeg: unit = (group,
 // segment of kTcSegTiles tiles); otherwise unit = (group, tile).  A new group's first K tile is requested
 // before the Q buffer is waited for, so it is in flight while the old group's MMAs drain.
 template <bool kSeg, bool kTrace>
 __device__ inline void tc_producer(const TcSmem& s, const TcBars& b, const CUtensorMap* tq, const CUtensorMap* tk,
-                                   const TcArgs& a, int u0, int u1) {
+                                   const TcArgs& a, int u0, int u1, TcRole& st, long long* trace_p) {
   const int upg = kSeg ? a.spg : a.tpg;
-  int ks = 0, kph = 0, n_q = 0, trace_n = 0;
+  int ks = st.ks, kph = st.kph, n_q = st.n_q, trace_n = 0;
   bool new_group = true;
   int x = u0 % upg;
   TcCursor g; g.init(a, u0 / upg);
@@ -159,6 +167,7 @@ __device__ inline void tc_producer(const TcSmem& s, const TcBars& b, const CUten
     }
     if (++x == upg) { x = 0; g.next(a); new_group = true; }
   }
+  st.ks = ks; st.kph = kph; st.n_q = n_q;
 }
 
 // =====================================================================================================
@@ -168,27 +177,21 @@ __device__ inline void tc_producer(const TcSmem& s, const TcBars& b, const CUten
 // (row block rbl, 64-token half th, lane quarter lg) takes its 64 columns as two 32-column blocks.
 // =====================================================================================================
 template <int kVar, bool kTrace>
-__global__ void __launch_bounds__(kTcThreads, 1)
-k_tc_stats(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k, TcArgs a) {
-  extern __shared__ uint8_t smem_raw[];
-  const TcSmem s = tc_carve(smem_raw, a);
-  const TcBars b = tc_bars(s);
+__device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const CUtensorMap* tmap_q, const CUtensorMap* tmap_k,
+                                         const TcArgs& a, uint32_t tmem_base, TcRole& st) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int U = a.n_groups * a.spg;                                      // schedule unit = (group, segment)
   const int s0 = tc_unit_begin(U, gridDim.x, blockIdx.x), s1 = tc_unit_begin(U, gridDim.x, blockIdx.x + 1);
-  if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.trace[4 * kTcTraceN + 2 * blockIdx.x] = t; }
-  const uint32_t tmem_base = tc_prologue(s, b, a, &tmap_q, &tmap_k);
-  pdl_wait();                       // the chunk's K rows come from k_append
-  if (threadIdx.x == 0) pdl_launch_dependents();
+  long long* const trace_p = a.trace;
 
   if (warp == 0) {
-    if (lane == 0) tc_producer<true, kTrace>(s, b, &tmap_q, &tmap_k, a, s0, s1);
+    if (lane == 0) tc_producer<true, kTrace>(s, b, tmap_q, tmap_k, a, s0, s1, st, trace_p);
   } else if (warp == 1) {
     // ---------------- MMA issuer: the whole warp runs the loop, one elected lane issues ----------------
     const uint32_t idesc = ptx::idesc_bf16_f32(128, kTcTile);
     const uint32_t q_lo = ptx::smem_desc_lo(ptx::smem_u32(s.q)), k_lo = ptx::smem_desc_lo(ptx::smem_u32(s.k));
     const uint32_t q_half16 = uint32_t(a.q_half_bytes) >> 4;
-    int ks = 0, kph = 0, as = 0, aph = 0, n_q = 0, trace_n = 0;
+    int ks = st.ks, kph = st.kph, as = st.as, aph = st.aph, n_q = st.n_q, trace_n = 0;
     bool new_group = true;
     int x = s0 % a.spg;
     TcCursor g; g.init(a, s0 / a.spg);
@@ -233,11 +236,12 @@ k_tc_stats(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ C
       }
       if (++x == a.spg) { x = 0; g.next(a); new_group = true; }
     }
+    st.ks = ks; st.kph = kph; st.as = as; st.aph = aph; st.n_q = n_q;
   } else {
     // ---------------- epilogue: one probe row x 64 tokens per thread per stage ----------------
     const int e = warp - 2, rbl = e >> 3, th = (e >> 2) & 1, lg = warp & 3;
     const uint32_t t_addr = tmem_base + (uint32_t(lg * 32) << 16) + rbl * kTcTile + th * 64;
-    int as = 0, aph = 0, trace_n = 0;
+    int as = st.as, aph = st.aph, trace_n = 0;
     const int trole = e == 0 ? 2 : 3;
     const bool tr = kTrace && lane == 0 && (e == 0 || e == kTcEpiWarps - 1);
     float m0 = -INFINITY, z0 = 0.f, m1 = -INFINITY, z1 = 0.f;            // running (max, sum) per half-group
@@ -273,8 +277,15 @@ k_tc_stats(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ C
       z_run = z_run * fast_exp2(m_run - m_new) + ((sm[0] + sm[1]) + (sm[2] + sm[3]));
       m_run = m_new;
     };
-    int x = s0 % a.spg;
-    TcCursor g; g.init(a, s0 / a.spg);
+    int x = s0 % a.spg, gi = s0 / a.spg, n_done = 0;
+    TcCursor g; g.init(a, gi);
+    // tell pass 2 (of this or a neighbouring CTA) that `n_done` more segments of group gi are in memory
+    auto publish = [&]() {
+      __threadfence();
+      __syncwarp();
+      if (lane == 0) atomicAdd(a.seg_cnt + gi, unsigned(n_done));
+      n_done = 0;
+    };
     for (int u = s0; u < s1; ++u) {
       const int rs_valid = g.rs_valid(a);
       const bool two = rs_valid > 256;                                   // the group has a second half-group
@@ -303,22 +314,32 @@ k_tc_stats(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ C
           if (tr) TC_TRACE(trole, 3);
         }
       }
-      // segment done: one partial per (segment, token half, row); rows / halves that saw no token write (-inf, 0)
+      // segment done: the two token-half warps of a (row block, lane quarter) merge through shared memory
+      // (double-buffered by segment parity, one 64-thread barrier), then one partial per (segment, row)
       {
-        float2* part = reinterpret_cast<float2*>(a.g.partial) +
-                       (size_t(g.bl(a)) * (2 * a.spg) + 2 * x + th) * (a.g.Hq * a.g.p_max) + g.stat_row0(a);
-        const int row_a = rbl * 128 + lg * 32 + lane, row_b = row_a + 256;
-        if (row_a < rs_valid) part[row_a] = make_float2(m0, z0);
-        if (row_b < rs_valid) part[row_b] = make_float2(m1, z1);
+        const int pair = rbl * 4 + lg;
+        float4* xch = s.xch + ((u & 1) * 8 + pair) * 32 + lane;
+        if (th == 1) *xch = make_float4(m0, z0, m1, z1);
+        ptx::named_bar_sync(2 + pair, 64);
+        if (th == 0) {
+          const float4 o = *xch;
+          const float ma = fmaxf(m0, o.x), mb = fmaxf(m1, o.z);            // this half always saw a token: finite
+          const float za = z0 * fast_exp2(m0 - ma) + o.y * fast_exp2(o.x - ma);
+          const float zb = z1 * fast_exp2(m1 - mb) + o.w * fast_exp2(o.z - mb);
+          float2* part = reinterpret_cast<float2*>(a.g.partial) +
+                         (size_t(g.bl(a)) * a.spg + x) * (a.g.Hq * a.g.p_max) + g.stat_row0(a);
+          const int row_a = rbl * 128 + lg * 32 + lane, row_b = row_a + 256;
+          if (row_a < rs_valid) part[row_a] = make_float2(ma, za);
+          if (row_b < rs_valid) part[row_b] = make_float2(mb, zb);
+        }
         m0 = m1 = -INFINITY; z0 = z1 = 0.f;
       }
-      if (++x == a.spg) { x = 0; g.next(a); }
+      ++n_done;
+      if (++x == a.spg) { publish(); x = 0; ++gi; g.next(a); }
     }
+    if (n_done > 0) publish();
+    st.as = as; st.aph = aph;
   }
-  ptx::tc_fence_before();
-  __syncthreads();
-  if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.trace[4 * kTcTraceN + 2 * blockIdx.x + 1] = t; }
-  if (warp == 1) ptx::tmem_dealloc(tmem_base, 512);
 }
 
 // Pass-2 group prologue: merges each probe row's per-(segment, half) (m, z) partials of pass 1 in slot
@@ -357,26 +378,20 @@ __device__ __noinline__ void tc_merge_rows(const float2* pr, int n_slot, int row
 // quarter cq) takes 32-column blocks cq and cq + 4 of the chunk.
 // =====================================================================================================
 template <int kVar, bool kTrace>
-__global__ void __launch_bounds__(kTcThreads, 1)
-k_tc_colsum(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k, TcArgs a) {
-  extern __shared__ uint8_t smem_raw[];
-  const TcSmem s = tc_carve(smem_raw, a);
-  const TcBars b = tc_bars(s);
+__device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const CUtensorMap* tmap_q, const CUtensorMap* tmap_k,
+                                         const TcArgs& a, uint32_t tmem_base, TcRole& st) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int U = a.n_groups * a.tpg;
   const int u0 = tc_unit_begin(U, gridDim.x, blockIdx.x), u1 = tc_unit_begin(U, gridDim.x, blockIdx.x + 1);
-  if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.trace[4 * kTcTraceN + 2 * blockIdx.x] = t; }
-  const uint32_t tmem_base = tc_prologue(s, b, a, &tmap_q, &tmap_k);
-  if (threadIdx.x == 0) pdl_launch_dependents();
-  // producer and MMA warps start at once (K and Q do not depend on pass 1); the epilogue waits for pass 1
+  long long* const trace_p = a.trace ? a.trace + kTcTraceStride : nullptr;
 
   if (warp == 0) {
-    if (lane == 0) tc_producer<false, kTrace>(s, b, &tmap_q, &tmap_k, a, u0, u1);
+    if (lane == 0) tc_producer<false, kTrace>(s, b, tmap_q, tmap_k, a, u0, u1, st, trace_p);
   } else if (warp == 1) {
     // ---------------- MMA issuer: the whole warp runs the loop, one elected lane issues ----------------
     const uint32_t q_lo = ptx::smem_desc_lo(ptx::smem_u32(s.q)), k_lo = ptx::smem_desc_lo(ptx::smem_u32(s.k));
     const uint32_t q_half16 = uint32_t(a.q_half_bytes) >> 4;
-    int ks = 0, kph = 0, as = 0, aph = 0, n_q = 0, trace_n = 0;
+    int ks = st.ks, kph = st.kph, as = st.as, aph = st.aph, n_q = st.n_q, trace_n = 0;
     bool new_group = true;
     int t = u0 % a.tpg;
     TcCursor g; g.init(a, u0 / a.tpg);
@@ -415,19 +430,18 @@ k_tc_colsum(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ 
     }
   } else {
     // ---------------- epilogue: one token per thread; warp (lane quarter lg, column quarter cq) ----------------
-    pdl_wait();
     const int e = warp - 2, cq = e >> 2, lg = warp & 3;
     const int tok_in_tile = lg * 32 + lane;
     const uint32_t t_addr = tmem_base + (uint32_t(lg * 32) << 16) + cq * 32;
-    int as = 0, aph = 0, trace_n = 0;
+    int as = st.as, aph = st.aph, trace_n = 0;
     const int trole = e == 0 ? 2 : 3;
     const bool tr = kTrace && lane == 0 && (e == 0 || e == kTcEpiWarps - 1);
     float v[32];
     float acc[4] = {0.f, 0.f, 0.f, 0.f};
     bool new_group = true;
-    int t = u0 % a.tpg, rs32 = 0;
+    int t = u0 % a.tpg, rs32 = 0, gi = u0 / a.tpg;
     float* col = nullptr;                                                // this warp's column-sum slot of the group
-    TcCursor g; g.init(a, u0 / a.tpg);
+    TcCursor g; g.init(a, gi);
     // sum over the 32 probe rows [col0, col0 + 32) of this token (32 registers live: no spills in this loop --
     // a local-memory load would queue behind the exp2 traffic like every other MIO instruction)
     auto fold = [&](int col0) {
@@ -458,11 +472,19 @@ k_tc_colsum(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ 
     };
     for (int u = u0; u < u1; ++u) {
       if (new_group) {
+        // all pass-1 segments of the group must be in memory (they come from this CTA and its schedule
+        // neighbours, none of which ever waits during pass 1, and every CTA of the grid is resident)
+        if (lane == 0) {
+          unsigned seen;
+          do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(a.seg_cnt + gi) : "memory"); }
+          while (int(seen - a.seg_target) < 0);
+        }
+        __syncwarp();
         ptx::named_bar_sync(1, kTcEpiWarps * 32);                        // everyone is done with the old c_r
         if (tr) TC_TRACE(trole, 5);
         const int bl = g.bl(a), rows_total = a.g.Hq * a.g.p_max;
-        tc_merge_rows(reinterpret_cast<const float2*>(a.g.partial) + size_t(bl) * (2 * a.spg) * rows_total + g.stat_row0(a),
-                      2 * a.spg, rows_total, g.rs_valid(a), s.c, threadIdx.x - 64);
+        tc_merge_rows(reinterpret_cast<const float2*>(a.g.partial) + size_t(bl) * a.spg * rows_total + g.stat_row0(a),
+                      a.spg, rows_total, g.rs_valid(a), s.c, threadIdx.x - 64);
         ptx::named_bar_sync(1, kTcEpiWarps * 32);
         if (tr) TC_TRACE(trole, 6);
         rs32 = (g.rs_valid(a) + 31) & ~31;
@@ -496,13 +518,36 @@ k_tc_colsum(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ 
       const int tok = t * kTcTile + tok_in_tile;
       if (tok < a.Tn) col[tok] = (acc[0] + acc[1]) + (acc[2] + acc[3]);
       acc[0] = acc[1] = acc[2] = acc[3] = 0.f;
-      if (++t == a.tpg) { t = 0; g.next(a); new_group = true; }
+      if (++t == a.tpg) { t = 0; ++gi; g.next(a); new_group = true; }
     }
   }
+}
+
+// =====================================================================================================
+// One persistent kernel runs both passes: every CTA works through its pass-1 range, then its pass-2
+// range of the same flattened (group, token) space, keeping TMEM, barriers and the K ring alive.  Pass 2
+// of a group only waits (on seg_cnt) for the pass-1 segments of that group, i.e. for this CTA and its
+// schedule neighbours -- there is no grid-wide barrier.  Requires gridDim.x <= #SMs (all CTAs resident).
+// =====================================================================================================
+template <int kVar, bool kTrace>
+__global__ void __launch_bounds__(kTcThreads, 1)
+k_tc_score(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k, TcArgs a) {
+  extern __shared__ uint8_t smem_raw[];
+  const TcSmem s = tc_carve(smem_raw, a);
+  const TcBars b = tc_bars(s);
+  if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.trace[4 * kTcTraceN + 2 * blockIdx.x] = t; }
+  const uint32_t tmem_base = tc_prologue(s, b, a, &tmap_q, &tmap_k);
+  pdl_wait();                       // the chunk's K rows come from k_append
+  if (threadIdx.x == 0) pdl_launch_dependents();
+  TcRole st;
+  tc_pass1<kVar, kTrace>(s, b, &tmap_q, &tmap_k, a, tmem_base, st);
+  if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.trace[4 * kTcTraceN + 2 * blockIdx.x + 1] = t; }
+  if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.trace[kTcTraceStride + 4 * kTcTraceN + 2 * blockIdx.x] = t; }
+  tc_pass2<kVar, kTrace>(s, b, &tmap_q, &tmap_k, a, tmem_base, st);
   ptx::tc_fence_before();
   __syncthreads();
-  if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.trace[4 * kTcTraceN + 2 * blockIdx.x + 1] = t; }
-  if (warp == 1) ptx::tmem_dealloc(tmem_base, 512);
+  if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.trace[kTcTraceStride + 4 * kTcTraceN + 2 * blockIdx.x + 1] = t; }
+  if ((threadIdx.x >> 5) == 1) ptx::tmem_dealloc(tmem_base, 512);
 }
 
 }  // namespace hk
@@ -522,8 +567,8 @@ struct TcState {
   int n_sm = 0;
   long long* trace = nullptr;   // 2 kernels x 4 roles x kTcTraceN events (HERMES_TC_TRACE=<file>)
   std::string trace_path;
-  void (*k_stats)(CUtensorMap, CUtensorMap, TcArgs) = nullptr;
-  void (*k_colsum)(CUtensorMap, CUtensorMap, TcArgs) = nullptr;
+  void (*k_score)(CUtensorMap, CUtensorMap, TcArgs) = nullptr;
+  unsigned seg_total = 0;       // running target of the pass-1 progress counters (wraps; compared wrap-safe)
   int var1 = 0, var2 = 0;   // experiment switches (HERMES_TC_VAR1 / HERMES_TC_VAR2)
 };
 
@@ -565,18 +610,13 @@ inline bool tc_init(hermes_t* h) {
   if (!tc_make_map(st, &st->tmap_k, g.kc, uint64_t(g.row_elems), uint64_t(g.B) * g.L * 2 * g.cap)) {
     h->err = "cuTensorMapEncodeTiled(K cache) failed"; delete st; return false;
   }
-  auto pick1 = [](int v) -> void (*)(CUtensorMap, CUtensorMap, TcArgs) {
-    switch (v) { case 1: return k_tc_stats<1, false>; case 3: return k_tc_stats<3, false>; case 5: return k_tc_stats<5, false>;
-                 case 7: return k_tc_stats<7, false>; case 9: return k_tc_stats<9, false>; default: return k_tc_stats<0, false>; }
+  auto pick = [](int v) -> void (*)(CUtensorMap, CUtensorMap, TcArgs) {
+    switch (v) { case 1: return k_tc_score<1, false>; case 3: return k_tc_score<3, false>; default: return k_tc_score<0, false>; }
   };
-  auto pick2 = [](int v) -> void (*)(CUtensorMap, CUtensorMap, TcArgs) {
-    switch (v) { case 1: return k_tc_colsum<1, false>; case 3: return k_tc_colsum<3, false>; case 5: return k_tc_colsum<5, false>;
-                 case 7: return k_tc_colsum<7, false>; case 9: return k_tc_colsum<9, false>; default: return k_tc_colsum<0, false>; }
-  };
-  st->k_stats = st->trace ? k_tc_stats<0, true> : pick1(st->var1);
-  st->k_colsum = st->trace ? k_tc_colsum<0, true> : pick2(st->var2);
-  if (cudaFuncSetAttribute(st->k_stats, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemMax) != cudaSuccess ||
-      cudaFuncSetAttribute(st->k_colsum, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemMax) != cudaSuccess) {
+  st->k_score = st->trace ? k_tc_score<0, true> : pick(st->var1);
+  int occ = 0;
+  if (cudaFuncSetAttribute(st->k_score, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemMax) != cudaSuccess ||
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, st->k_score, kTcThreads, kTcSmemMax) != cudaSuccess || occ < 1) {
     h->err = std::string("cudaFuncSetAttribute(tc kernels): ") + cudaGetErrorString(cudaGetLastError());
     delete st; return false;
   }
@@ -630,22 +670,22 @@ inline int tc_score(hermes_t* h, const void* q_probe, int Tn, int P, float scale
   a.spg = (a.tpg + kTcSegTiles - 1) / kTcSegTiles;
   const long long U1 = (long long)a.n_groups * a.spg, U2 = (long long)a.n_groups * a.tpg;
   if (U2 > INT_MAX / 2) { h->err = "tcgen05 scoring: too many (group, tile) units"; return HERMES_ECAPACITY; }
-  const int n_cta1 = int(std::min<long long>(st->n_sm, U1)), n_cta2 = int(std::min<long long>(st->n_sm, U2));
-  if (2 * a.spg > h->lay.n_part_max || g.Hkv * a.n_sc * 4 > g.n_vh_max) { h->err = "internal: tc scratch too small"; return HERMES_ESTATE; }
+  // every CTA must be resident (pass 2 waits on pass-1 progress of other CTAs): at most one CTA per SM
+  const int n_cta = int(std::min<long long>(st->n_sm, U1));
+  if (a.spg > h->lay.n_part_max || g.Hkv * a.n_sc * 4 > g.n_vh_max) { h->err = "internal: tc scratch too small"; return HERMES_ESTATE; }
   h->n_vh = g.Hkv * a.n_sc * 4;
   a.q_half_bytes = (a.RS + 63) / 64 * 8192;
   a.n_kst = std::min(kTcKStagesMax, (kTcSmemMax - tc_smem_bytes(a.q_half_bytes, 0)) / kTcKStage);
   const int smem = tc_smem_bytes(a.q_half_bytes, a.n_kst);
+  st->seg_total += unsigned(a.spg) * kTcEpiWarps;
+  a.seg_cnt = reinterpret_cast<unsigned*>(h->ws + h->lay.seg_cnt);
+  a.seg_target = st->seg_total;
   {
     TcProf p(h, HERMES_K_SCORE_STATS, s);
     a.trace = st->trace;
     if (st->trace) cudaMemsetAsync(st->trace, 0, 2 * kTcTraceStride * 8, s);
-    launch_pdl(st->k_stats, dim3(n_cta1), dim3(kTcThreads), size_t(smem), s, tmap_q, st->tmap_k, a);
-  }
-  {
-    TcProf p(h, HERMES_K_SCORE_COLSUM, s);
-    a.trace = st->trace ? st->trace + kTcTraceStride : nullptr;
-    launch_pdl(st->k_colsum, dim3(n_cta2), dim3(kTcThreads), size_t(smem), s, tmap_q, st->tmap_k, a);
+    const cudaError_t e = launch_pdl(st->k_score, dim3(n_cta), dim3(kTcThreads), size_t(smem), s, tmap_q, st->tmap_k, a);
+    if (e != cudaSuccess) { h->err = std::string("tcgen05 scoring launch: ") + cudaGetErrorString(e); return HERMES_ECUDA; }
   }
   return HERMES_OK;
 }
