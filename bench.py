@@ -22,7 +22,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from workloads import CONFIGS, chunk_kv, probe_q  # noqa: E402
+from workloads import CONFIGS, chunk_kv, probe_q, sweep_point  # noqa: E402
 
 METRIC, UNIT = "kv_tokens_managed_per_s", "tokens/s"
 POOL = 16          # distinct pre-generated chunk/probe sets cycled through the timed region
@@ -88,6 +88,18 @@ class ClockSampler:
                 "power_w_max": max(float(r[2]) for r in rows), "reasons": reasons}
 
 
+def workload_by_name(name: str):
+    """CONFIGS key, or `sweep:<budget>:<probe>` for a point of BASELINE.json configs[3]."""
+    if name.startswith("sweep:"):
+        _, m, p = name.split(":")
+        return sweep_point(int(m), int(p))
+    return CONFIGS[name]
+
+
+def cfg_index(name: str) -> int:
+    return 3 if name.startswith("sweep") else {"toy": 0, "llava_ov_7b": 1, "qwen25_vl_7b": 2, "batched_72b": 4}[name]
+
+
 def dist_env():
     return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
 
@@ -132,19 +144,22 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    wl = CONFIGS[args.workload]
+    wl = workload_by_name(args.workload)
     B = wl.n_streams
     tdt = torch.bfloat16 if wl.dtype == "bf16" else torch.float32
-    cfg = hb.config_for_workload(wl, device=local_rank)
+    cfg = hb.config_for_workload(wl, device=local_rank, score_path={"auto": 0, "simt": 1, "tcgen05": 2}[args.score_path])
     h = hb.hermes_create(cfg)
 
     host_pool = [tuple(torch.from_numpy(x).to(tdt).pin_memory() for x in s) for s in make_pool(wl, rank, POOL)]
     dev_pool = [tuple(x.to(dev) for x in s) for s in host_pool]
     # fill to the budget without a probe (no eviction), then W warm evicting updates
-    n_fill = wl.budget // wl.chunk_tokens
+    n_fill, rem = divmod(wl.budget, wl.chunk_tokens)
     for i in range(n_fill):
         K, V, _ = dev_pool[i % POOL]
         hb.hermes_append_chunk(h, K, V, None)
+    if rem:                                                  # budget not a multiple of the chunk: one partial append
+        K, V, _ = dev_pool[n_fill % POOL]
+        hb.hermes_append_chunk(h, K[:, :, :rem].contiguous(), V[:, :, :rem].contiguous(), None)
     assert hb.hermes_len(h) == wl.budget
 
     def barrier():
@@ -204,6 +219,9 @@ def run_ours(args):
         hb.hermes_destroy(h)
         return None
     work = algorithmic_work(wl, B)
+    row_b = wl.n_kv_heads * wl.head_dim * (2 if wl.dtype == "bf16" else 4)
+    ws_mb = B * wl.n_layers * 2 * work["T"] * row_b / 1e6          # K and V slabs read (scoring + gather)
+    wr_mb = B * wl.n_layers * 2 * wl.budget * row_b / 1e6            # compacted K and V written
     pk = peaks()
     sm = clocks.get("sm_mhz") if clocks else None
     kern = {k: v for k, v in acc.items() if v > 0}
@@ -242,11 +260,13 @@ def run_ours(args):
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "chunk_update_latency_us": ms * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": wl.dtype, "data": "synthetic",
-        "config": {"workload": f"BASELINE.json configs[1] {wl.name}: L{wl.n_layers} Hq{wl.n_q_heads}/Hkv{wl.n_kv_heads} "
+        "config": {"workload": f"BASELINE.json configs[{cfg_index(wl.name)}] {wl.name}: L{wl.n_layers} Hq{wl.n_q_heads}/Hkv{wl.n_kv_heads} "
                                f"d{wl.head_dim} {wl.dtype}, budget {wl.budget}, chunk {wl.chunk_tokens}, probe {wl.probe_tokens}, "
                                f"T {work['T']}", "streams_per_gpu": B, "parallelism": f"replicas x{world} (independent streams, no collective)",
-                   "l2": "working set per step (K+V read 370 MB + 360 MB written) exceeds the 126 MB L2; inputs cycle through "
-                         f"{POOL} chunk/probe sets", "score_path": score_path},
+                   "l2": (f"cache slabs touched per step: {ws_mb:.0f} MB read + {wr_mb:.0f} MB written "
+                          + ("(exceeds the 126 MB L2)" if ws_mb + wr_mb > 252 else "(comparable to the 126 MB L2: no flush, L2-assisted)")
+                          + f"; inputs cycle through {POOL} chunk/probe sets"),
+                   "score_path": score_path},
         "e2e": {"value": job_value(wl, world, B, ms_e2e), "unit": UNIT, "ms_per_step": ms_e2e,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e},
         "gpu_launches": launches,
@@ -292,7 +312,7 @@ def run_reference(args):
     rank, _, world = dist_env()
     if rank != 0:
         return None
-    wl = CONFIGS[args.workload]
+    wl = workload_by_name(args.workload)
     Ls = 4                                                   # 1 shallow + 2 middle + 1 deep (10/60/30 % rule at L = 4)
     sec, threads, swl = oracle_sample(wl, args.steps, Ls, warmup=min(args.warmup, 2))
     T = wl.budget + wl.chunk_tokens
@@ -313,7 +333,8 @@ def main():
     ap.add_argument("--steps", type=int, default=1024)
     ap.add_argument("--warmup", type=int, default=8)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="llava_ov_7b", choices=sorted(CONFIGS))
+    ap.add_argument("--workload", default="llava_ov_7b", help="one of %s, or sweep:<budget>:<probe>" % sorted(CONFIGS))
+    ap.add_argument("--score-path", default="auto", choices=["auto", "simt", "tcgen05"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -322,7 +343,7 @@ def main():
         out = run_ours(args)
         rank, _, world = dist_env()
         if out is not None and world == 1 and not args.no_cpu_baseline:
-            wl = CONFIGS[args.workload]
+            wl = workload_by_name(args.workload)
             sec, threads, swl = oracle_sample(wl, 2, wl.n_layers)       # two full-size oracle updates
             T = wl.budget + wl.chunk_tokens
             out["cpu_baseline"] = {"value": wl.n_layers * T / sec, "unit": UNIT, "cores": threads, "kind": "oracle",

@@ -70,6 +70,9 @@ class OracleConfig:
     mrope_grid_h: int = 8
     mrope_grid_w: int = 8
     pos_offset: int = 0               # length of the fixed system prefix
+    reindex_mode: str = "eager"       # "eager" | "lazy" (DESIGN f2)
+    max_position: int = 0             # lazy: the model's position limit that triggers a re-index
+    max_chunk_span: int = 0           # lazy: largest position span of one arriving chunk (tokens; M-RoPE: t steps)
     capacity: int = 0                 # slots per layer; 0 -> budget + largest chunk seen
 
     @property
@@ -301,6 +304,7 @@ class OracleStream:
     pos: Optional[np.ndarray] = None
     len: int = 0
     t_steps_seen: int = 0             # M-RoPE: temporal steps appended so far
+    next_pos: int = -1                # lazy mode: position (1D) / temporal index (M-RoPE) after the newest token
     last: dict = field(default_factory=dict)
 
     def _ensure(self, need: int):
@@ -327,15 +331,24 @@ def arrival_positions(cfg: OracleConfig, st: OracleStream, n_new: int, pos_start
     default first step = offset + min(steps seen, |M|), which is host-computable and
     above every compacted t of every layer (DESIGN c13/c16)."""
     j = np.arange(n_new, dtype=np.int64)
+    lazy = cfg.reindex_mode == "lazy"
+    nxt = st.next_pos if st.next_pos >= 0 else cfg.pos_offset       # lazy: positions keep growing (PAPER.md:126-128)
     if cfg.rope_mode == "1d":
-        p0 = pos_start if pos_start >= 0 else cfg.pos_offset + st.len
+        p0 = pos_start if pos_start >= 0 else (nxt if lazy else cfg.pos_offset + st.len)
         return (p0 + j)[None, :]
     tpt = cfg.mrope_grid_h * cfg.mrope_grid_w
-    t0 = pos_start if pos_start >= 0 else cfg.pos_offset + min(st.t_steps_seen, cfg.budget)
+    t0 = pos_start if pos_start >= 0 else (nxt if lazy else cfg.pos_offset + min(st.t_steps_seen, cfg.budget))
     t = t0 + j // tpt
     h = cfg.pos_offset + (j % tpt) // cfg.mrope_grid_w
     w = cfg.pos_offset + j % cfg.mrope_grid_w
     return np.stack([t, h, w])
+
+
+def lazy_reindex_due(cfg: OracleConfig, p_end: int) -> bool:
+    """Lazy re-indexing: re-index "only when positional indices approach the model limit".
+    Reading (DESIGN f2): the compression step re-indexes when the NEXT chunk (at most `max_chunk_span`
+    positions) would no longer fit below `max_position`, p_end being the position after the newest token."""
+    return p_end + cfg.max_chunk_span > cfg.max_position
 
 
 def oracle_step(st: OracleStream, K_new: np.ndarray, V_new: np.ndarray,
@@ -357,9 +370,13 @@ def oracle_step(st: OracleStream, K_new: np.ndarray, V_new: np.ndarray,
     st.K[:, st.len:T] = K_new
     st.V[:, st.len:T] = V_new
     st.pos[:, :, st.len:T] = p_arr[None, :, :]
+    span = n_new
     if cfg.rope_mode == "m3d":
         tpt = cfg.mrope_grid_h * cfg.mrope_grid_w
-        st.t_steps_seen += (n_new + tpt - 1) // tpt
+        span = (n_new + tpt - 1) // tpt
+        st.t_steps_seen += span
+    p_end = int(p_arr[0, 0]) + span                    # position after the newest token (t axis for M-RoPE)
+    st.next_pos = p_end
     if Q_probe is None or T <= cfg.budget:        # "triggered once the budget is exceeded"
         st.len = T
         st.last = {"T": T, "evicted": False}
@@ -381,10 +398,11 @@ def oracle_step(st: OracleStream, K_new: np.ndarray, V_new: np.ndarray,
     pos_new = np.zeros((L, cfg.n_axes, cfg.budget), np.int64)
     K_out = np.zeros((L, cfg.budget) + st.K.shape[2:], np.float32)
     V_out = np.zeros_like(K_out)
+    reindex = cfg.reindex_mode == "eager" or lazy_reindex_due(cfg, p_end)
     for l in range(L):
         I = select_topk(S_tilde[l], cfg.budget)
         p_old = st.pos[l][:, I]
-        p_new = compact_positions(cfg, p_old)
+        p_new = compact_positions(cfg, p_old) if reindex else p_old   # lazy: keep the original indices
         kept[l], pos_new[l] = I, p_new
         V_out[l] = st.V[l, I]                                  # V_l[I_l], bit for bit
         K_out[l] = rotary_delta(cfg, st.K[l, I], p_new - p_old)
@@ -392,6 +410,8 @@ def oracle_step(st: OracleStream, K_new: np.ndarray, V_new: np.ndarray,
     st.V[:, :cfg.budget] = V_out
     st.pos[:, :, :cfg.budget] = pos_new
     st.len = cfg.budget                                        # 9.
-    st.last = {"T": T, "evicted": True, "W": W, "S": S, "S_tilde": S_tilde,
+    if reindex:                       # every position is now below offset + |M| (M-RoPE: + min(steps seen, |M|))
+        st.next_pos = cfg.pos_offset + (cfg.budget if cfg.rope_mode == "1d" else min(st.t_steps_seen, cfg.budget))
+    st.last = {"T": T, "evicted": True, "reindexed": reindex, "W": W, "S": S, "S_tilde": S_tilde,
                "kept": kept, "pos_new": pos_new}
     return st.last
