@@ -49,6 +49,7 @@ enum { HERMES_F32 = 0, HERMES_BF16 = 1 };
 enum { HERMES_ROPE_1D = 0, HERMES_ROPE_M3D = 1 };   /* App. E.1 / App. E.2                    */
 enum { HERMES_NORM_MAX = 0, HERMES_NORM_SUM = 1 };  /* alpha of Eq. 1/2 (DESIGN c2)           */
 enum { HERMES_SCORE_AUTO = 0, HERMES_SCORE_SIMT = 1, HERMES_SCORE_TCGEN05 = 2 };
+enum { HERMES_REINDEX_EAGER = 0, HERMES_REINDEX_LAZY = 1 };   /* Sec. 3.3   */
 
 typedef struct hermes hermes_t;  /* opaque; owns n_streams x n_layers double-buffered caches   */
 
@@ -75,6 +76,11 @@ typedef struct {
   int32_t mrope_compact_axes;   /* bit0 t, bit1 h, bit2 w: axes re-indexed by Eq. 11           */
   int32_t mrope_grid_h, mrope_grid_w; /* merged patch grid; tokens per temporal step = h*w     */
   int32_t pos_offset;           /* length of the fixed system prefix            */
+  int32_t reindex_mode;         /* HERMES_REINDEX_*: EAGER re-indexes at every compression step;
+                                   LAZY keeps original indices (kept keys are copied, not rotated) and
+                                   re-indexes only at the step after which the next chunk (max_chunk_tokens
+                                   positions; M-RoPE: its temporal steps) would exceed max_position        */
+  int32_t max_position;         /* LAZY: the model's position limit (> pos_offset + budget + chunk span) */
   int32_t score_path;           /* HERMES_SCORE_*: AUTO picks tcgen05 when the contraction is dense */
   int32_t device;               /* CUDA device ordinal                                         */
 } hermes_config;

@@ -38,6 +38,7 @@ __all__ = [
     "lambda_of_layer", "attention_weights", "recency_scores", "normalise_attention",
     "raw_scores", "smooth_scores", "select_topk", "compact_positions",
     "rope_frequencies", "pair_axis", "rotary_delta", "round_to_storage", "oracle_step",
+    "summary_token", "lazy_reindex_due",
 ]
 
 
@@ -73,6 +74,7 @@ class OracleConfig:
     reindex_mode: str = "eager"       # "eager" | "lazy" (DESIGN f2)
     max_position: int = 0             # lazy: the model's position limit that triggers a re-index
     max_chunk_span: int = 0           # lazy: largest position span of one arriving chunk (tokens; M-RoPE: t steps)
+    summary_token: bool = False       # deep layers: evicted tokens -> one summary token (Alg. 1; DESIGN f1)
     capacity: int = 0                 # slots per layer; 0 -> budget + largest chunk seen
 
     @property
@@ -293,6 +295,30 @@ def rotary_delta(cfg: OracleConfig, k_old: np.ndarray, delta: np.ndarray) -> np.
     return np.where(zero2, k_old, out).astype(np.float32)
 
 
+def summary_token(cfg: OracleConfig, K_p: np.ndarray, V_p: np.ndarray, P_p: np.ndarray, t: int):
+    """Algorithm 1: one (k_sum, v_sum) from the pruned tokens of a layer.
+
+    K_p, V_p: [n, H_kv, d] pruned keys / values (storage values); P_p: [1, n] their position indices;
+    t: target position of the summary token.  Step 1: v_sum = Mean(V_p).  Step 2: every pruned key is
+    phase-aligned to t by the rotary delta t - p (Eq. 9-10, fp64 angle, fp32 cos / sin and rotation as in
+    `rotary_delta`, NOT rounded to storage), then k_sum = Mean(K_aligned).  Means are taken in fp64 and
+    rounded once to the storage dtype (DESIGN f1).  1D RoPE only."""
+    n, _, d = K_p.shape
+    half = d // 2
+    theta = rope_frequencies(d, cfg.rope_theta)
+    ang = (float(t) - P_p[0].astype(np.float64))[:, None] * theta[None, :]     # [n, half]
+    c = np.cos(ang).astype(np.float32)[:, None, :]
+    s_ = np.sin(ang).astype(np.float32)[:, None, :]
+    x = K_p[:, :, :half].astype(np.float32)
+    y = K_p[:, :, half:].astype(np.float32)
+    xa = ((x * c).astype(np.float32) - (y * s_).astype(np.float32)).astype(np.float32)
+    ya = ((x * s_).astype(np.float32) + (y * c).astype(np.float32)).astype(np.float32)
+    K_aligned = np.concatenate([xa, ya], axis=2).astype(np.float64)
+    k_sum = round_to_storage(K_aligned.mean(axis=0).astype(np.float32), cfg.dtype)
+    v_sum = round_to_storage(V_p.astype(np.float64).mean(axis=0).astype(np.float32), cfg.dtype)
+    return k_sum, v_sum
+
+
 # --------------------------------------------------------------------------- state + step
 @dataclass
 class OracleStream:
@@ -399,7 +425,25 @@ def oracle_step(st: OracleStream, K_new: np.ndarray, V_new: np.ndarray,
     K_out = np.zeros((L, cfg.budget) + st.K.shape[2:], np.float32)
     V_out = np.zeros_like(K_out)
     reindex = cfg.reindex_mode == "eager" or lazy_reindex_due(cfg, p_end)
+    if cfg.summary_token and (cfg.rope_mode != "1d" or cfg.reindex_mode != "eager"):
+        raise ValueError("summary tokens are defined here for eager 1D re-indexing only (DESIGN f1)")
     for l in range(L):
+        if cfg.summary_token and layer_stage(cfg, l) == "deep":
+            # deep layers keep |M| - 1 tokens by Top-K and append ONE summary token of everything evicted, so the
+            # layer still holds exactly |M| tokens; it sits after the kept tokens
+            # (Alg. 1 step 3) at the next contiguous position t = offset + |M| - 1 and is an ordinary,
+            # evictable token from then on (DESIGN f1).  kept[l][-1] = -1 marks it.
+            I = select_topk(S_tilde[l], cfg.budget - 1)
+            ev = np.setdiff1d(np.arange(T), I)
+            p_old = st.pos[l][:, I]
+            p_new = compact_positions(cfg, p_old)
+            t = cfg.pos_offset + cfg.budget - 1
+            k_sum, v_sum = summary_token(cfg, st.K[l, ev], st.V[l, ev], st.pos[l][:, ev], t)
+            kept[l, :-1], kept[l, -1] = I, -1
+            pos_new[l][:, :-1], pos_new[l][:, -1] = p_new, t
+            V_out[l, :-1], V_out[l, -1] = st.V[l, I], v_sum
+            K_out[l, :-1], K_out[l, -1] = rotary_delta(cfg, st.K[l, I], p_new - p_old), k_sum
+            continue
         I = select_topk(S_tilde[l], cfg.budget)
         p_old = st.pos[l][:, I]
         p_new = compact_positions(cfg, p_old) if reindex else p_old   # lazy: keep the original indices

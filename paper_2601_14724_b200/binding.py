@@ -15,6 +15,7 @@ from . import build as _build
 HERMES_OK, HERMES_EINVAL, HERMES_ECAPACITY, HERMES_ESTATE, HERMES_ECUDA, HERMES_ENOMEM = 0, -1, -2, -3, -4, -5
 HERMES_F32, HERMES_BF16 = 0, 1
 HERMES_ROPE_1D, HERMES_ROPE_M3D = 0, 1
+HERMES_REINDEX_EAGER, HERMES_REINDEX_LAZY = 0, 1
 HERMES_NORM_MAX, HERMES_NORM_SUM = 0, 1
 HERMES_SCORE_AUTO, HERMES_SCORE_SIMT, HERMES_SCORE_TCGEN05 = 0, 1, 2
 HERMES_K_NAMES = ("append", "score_stats", "score_combine", "score_colsum", "select", "gather")
@@ -35,7 +36,8 @@ class HermesConfig(C.Structure):
                 ("lambda_deep", C.c_float), ("softmax_scale", C.c_float), ("rope_mode", C.c_int32),
                 ("rope_theta", C.c_float), ("mrope_section", C.c_int32 * 3),
                 ("mrope_compact_axes", C.c_int32), ("mrope_grid_h", C.c_int32),
-                ("mrope_grid_w", C.c_int32), ("pos_offset", C.c_int32), ("score_path", C.c_int32),
+                ("mrope_grid_w", C.c_int32), ("pos_offset", C.c_int32), ("reindex_mode", C.c_int32),
+                ("max_position", C.c_int32), ("score_path", C.c_int32),
                 ("device", C.c_int32)]
 
 

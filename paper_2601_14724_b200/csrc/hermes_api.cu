@@ -43,6 +43,7 @@ extern "C" void hermes_default_config(hermes_config* c) {
   c->mrope_compact_axes = 1; c->mrope_grid_h = 8; c->mrope_grid_w = 8;
   c->max_probe_tokens = 64;
   c->score_path = HERMES_SCORE_AUTO;
+  c->reindex_mode = HERMES_REINDEX_EAGER;
 }
 
 extern "C" size_t hermes_workspace_bytes(const hermes_config* c) {
@@ -255,16 +256,24 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
   // arrival positions (DESIGN c16): host-computable, strictly above every cached position
   long long p0;
   long long steps = 0;
+  const bool lazy = c.reindex_mode == HERMES_REINDEX_LAZY;
+  long long span = n_new;                       // positions the chunk spans on the re-indexed axis
   if (g.n_axes == 1) {
-    p0 = pos_start >= 0 ? pos_start : c.pos_offset + h->len;
+    p0 = pos_start >= 0 ? pos_start : (lazy ? h->next_pos : c.pos_offset + h->len);
   } else {
     const int tpt = c.mrope_grid_h * c.mrope_grid_w;
     steps = (n_new + tpt - 1) / tpt;
-    p0 = pos_start >= 0 ? pos_start : c.pos_offset + std::min<long long>(h->t_steps_seen, c.budget);
+    span = steps;
+    p0 = pos_start >= 0 ? pos_start : (lazy ? h->next_pos : c.pos_offset + std::min<long long>(h->t_steps_seen, c.budget));
   }
   if (p0 < h->next_pos) return fail(h, HERMES_EINVAL, "pos_start %lld is not above the cached positions (need >= %lld)", p0, h->next_pos);
   if (p0 + std::max<long long>(n_new, steps) >= INT_MAX) return fail(h, HERMES_EINVAL, "position overflow");
   const bool evict = Q_probe != nullptr && Tn > c.budget;
+  // lazy mode: re-index only when the next chunk would no longer fit below max_position
+  const long long span_max = g.n_axes == 1 ? c.max_chunk_tokens
+                                           : (c.max_chunk_tokens + c.mrope_grid_h * c.mrope_grid_w - 1) / (c.mrope_grid_h * c.mrope_grid_w);
+  const bool reindex = !lazy || p0 + span + span_max > c.max_position;
+  if (lazy && p0 + span > c.max_position) return fail(h, HERMES_ECAPACITY, "positions would exceed max_position %d", c.max_position);
 
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   h->last_launches = 0;
@@ -301,7 +310,7 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
       const float r_norm_sum = float((1.0 - std::exp(-k)) / (1.0 - std::exp(-k * Tn)));
       if (g.L > g.n_shallow)
         launch_pdl(k_wsum, dim3((Tn + 255) / 256, g.B * (g.L - g.n_shallow)), dim3(256), 0, s, g, Tn, n_probe, h->n_vh);
-      launch_pdl(k_select, dim3(BL), dim3(kSelThreads), size_t(Tn) * 4, s, g, h->cur, Tn, c.forget_rate, int(c.norm_mode == HERMES_NORM_SUM), r_norm_sum);
+      launch_pdl(k_select, dim3(BL), dim3(kSelThreads), size_t(Tn) * 4, s, g, h->cur, Tn, c.forget_rate, int(c.norm_mode == HERMES_NORM_SUM), r_norm_sum, int(reindex));
     }
     {
       Prof p(h, HERMES_K_GATHER, s);
@@ -327,6 +336,7 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
   if (g.n_axes == 3) h->t_steps_seen += steps;
   if (evict) {
     h->cur ^= 1; h->len = c.budget; h->last_T = Tn;
+    if (!reindex) h->next_pos = p0 + span; else
     // after eager re-indexing every cached position is below offset + budget (1D) or below
     // offset + min(temporal steps seen, budget) (M-RoPE: a layer holds at most that many distinct t)
     h->next_pos = c.pos_offset + (g.n_axes == 1 ? (long long)c.budget : std::min<long long>(h->t_steps_seen, c.budget));

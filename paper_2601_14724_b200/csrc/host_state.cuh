@@ -56,6 +56,14 @@ inline const char* validate(const hermes_config& c) {
     if (c.mrope_compact_axes < 0 || c.mrope_compact_axes > 7) return "bad mrope_compact_axes";
   }
   if (c.pos_offset < 0) return "pos_offset must be >= 0";
+  if (c.reindex_mode != HERMES_REINDEX_EAGER && c.reindex_mode != HERMES_REINDEX_LAZY) return "bad reindex_mode";
+  if (c.reindex_mode == HERMES_REINDEX_LAZY) {
+    const long long span = c.rope_mode == HERMES_ROPE_M3D
+        ? (c.max_chunk_tokens + c.mrope_grid_h * c.mrope_grid_w - 1) / (c.mrope_grid_h * c.mrope_grid_w) : c.max_chunk_tokens;
+    if ((long long)c.max_position < (long long)c.pos_offset + c.budget + 2 * span)
+      return "lazy re-indexing needs max_position >= pos_offset + budget + 2 chunk spans";
+    if (c.max_position > (1 << 20)) return "max_position too large (rotary table)";
+  }
   if (c.score_path < HERMES_SCORE_AUTO || c.score_path > HERMES_SCORE_TCGEN05) return "bad score_path";
   if (size_t(c.budget) + size_t(c.max_chunk_tokens) > (size_t(1) << 24)) return "budget + chunk too large";
   return nullptr;
@@ -78,6 +86,8 @@ inline Layout make_layout(const hermes_config& c) {
   } else {
     y.table_rows = y.cap - c.budget + 1;
   }
+  // lazy mode: a re-index step moves positions from anywhere below the limit down to the compact range
+  if (c.reindex_mode == HERMES_REINDEX_LAZY) y.table_rows = std::max(y.table_rows, c.max_position - c.pos_offset + 2);
   const size_t BL = size_t(c.n_streams) * c.n_layers;
   const size_t rows = size_t(c.n_q_heads) * c.max_probe_tokens;
   size_t o = 0;

@@ -107,7 +107,7 @@ k_wsum(Geom g, int Tn, int P, int n_vh) {
 }
 
 __global__ void __launch_bounds__(kSelThreads)
-k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum) {
+k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum, int reindex) {
   extern __shared__ float s_sc[];                    // [Tn] smoothed scores
   // per-warp digit histograms (radix phase); the M-RoPE rank bitmap + word prefixes reuse the space later
   __shared__ __align__(16) int whist[32 * 256];
@@ -293,8 +293,9 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
         const int out = i - lt_before - min(eq_before, r_eq);            // slot of token i among the kept
         kept[out] = i;
         if (g.n_axes == 1) {                                             // Eq. 8: positions rise with the index -> rank = slot
-          pos_new[out] = g.pos_offset + out;
-          dl1[out] = g.pos_offset + out - p_old[j];
+          // lazy mode between re-index steps keeps the original index: delta 0 = bit-exact key copy
+          pos_new[out] = reindex ? g.pos_offset + out : p_old[j];
+          dl1[out] = reindex ? g.pos_offset + out - p_old[j] : 0;
         }
       }
     }
@@ -311,7 +312,7 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
     const int32_t* po = pos_old + size_t(a) * g.cap;
     int32_t* pn = pos_new + size_t(a) * g.cap;
     int32_t* dl = g.delta + (size_t(bl) * 3 + a) * g.budget;
-    if (!((g.compact_axes >> a) & 1)) {                 // axis kept as is (DESIGN c13)
+    if (!reindex || !((g.compact_axes >> a) & 1)) {     // axis kept as is (DESIGN c13; lazy mode between re-index steps)
       for (int s = tid; s < g.budget; s += kSelThreads) { pn[s] = __ldcg(po + kept[s]); dl[s] = 0; }
       continue;
     }

@@ -38,6 +38,7 @@ class LockStep:
         self.feeders = [Feeder(wl, b) for b in range(self.B)]
         self.checked_streams = list(range(self.B)) if streams is None else streams
         self.t_steps_seen = 0
+        self.next_pos = -1                      # lazy mode: mirrors the library's running position
         self.ids = [np.zeros((wl.n_layers, 0), np.int64) for _ in range(self.B)]
         self.report = []
 
@@ -59,12 +60,14 @@ class LockStep:
             st.pos[l, :, :n] = v["pos"].cpu().numpy()
         st.len = n
         st.t_steps_seen = self.t_steps_seen
+        st.next_pos = self.next_pos
         return st
 
     def _arrival(self, n_new, pos_start=-1):
         st = ho.OracleStream(self.ocfg)
         st.len = hb.hermes_len(self.h)
         st.t_steps_seen = self.t_steps_seen
+        st.next_pos = self.next_pos
         return ho.arrival_positions(self.ocfg, st, n_new, pos_start)
 
     def _gen(self, n_new, with_probe, n_probe=None, pos_start=-1):
@@ -74,10 +77,16 @@ class LockStep:
         Q = np.stack([p[2] for p in per]) if with_probe else None
         return K, V, Q, [p[3] for p in per]
 
-    def _after(self, n_new, new_ids, evicted):
+    def _after(self, n_new, new_ids, evicted, p0=0):
+        span = n_new
         if self.ocfg.rope_mode == "m3d":
             tpt = self.ocfg.mrope_grid_h * self.ocfg.mrope_grid_w
-            self.t_steps_seen += (n_new + tpt - 1) // tpt
+            span = (n_new + tpt - 1) // tpt
+            self.t_steps_seen += span
+        c = self.ocfg
+        self.next_pos = p0 + span
+        if evicted and (c.reindex_mode == "eager" or ho.lazy_reindex_due(c, p0 + span)):
+            self.next_pos = c.pos_offset + (c.budget if c.rope_mode == "1d" else min(self.t_steps_seen, c.budget))
         for b in range(self.B):
             self.ids[b] = np.concatenate([self.ids[b], np.broadcast_to(new_ids[b], (self.wl.n_layers, n_new))], 1)
         if evicted:
@@ -90,20 +99,22 @@ class LockStep:
     # ---- schedule -------------------------------------------------------------------------------
     def fill(self):
         for n in fill_chunks(self.wl):
+            p0 = int(self._arrival(n)[0, 0])
             K, V, _, ids = self._gen(n, False)
             hb.hermes_append_chunk(self.h, to_dev(K, self.wl.dtype), to_dev(V, self.wl.dtype), None)
-            self._after(n, ids, False)
+            self._after(n, ids, False, p0)
 
     def step(self, check=True, n_new=None, n_probe=None, pos_start=-1):
         wl = self.wl
         n_new = wl.chunk_tokens if n_new is None else n_new
+        p0 = int(self._arrival(n_new, pos_start)[0, 0])
         K, V, Q, ids = self._gen(n_new, True, n_probe, pos_start)
         pre = {b: self.gpu_state(b) for b in self.checked_streams} if check else {}
         T = hb.hermes_len(self.h) + n_new
         hb.hermes_append_chunk(self.h, to_dev(K, wl.dtype), to_dev(V, wl.dtype), to_dev(Q, wl.dtype), pos_start)
         torch.cuda.synchronize()
         evicted = T > wl.budget
-        self._after(n_new, ids, evicted)
+        self._after(n_new, ids, evicted, p0)
         results = []
         for b, st in pre.items():
             out = ho.oracle_step(st, K[b], V[b], Q[b], pos_start)

@@ -61,6 +61,13 @@ class Feeder:
         return K, V, Q, ids
 
 
+def take_ids(ids: np.ndarray, kept: np.ndarray) -> np.ndarray:
+    """Token ids of the kept slots; kept == -1 (a summary token, DESIGN f1) gets id -1."""
+    out = np.take_along_axis(ids, np.maximum(kept, 0), axis=1)
+    out[kept < 0] = -1
+    return out
+
+
 def fill_chunks(wl: Workload):
     """Chunk sizes of the un-probed fill phase: preload (config 1) or chunks up to the budget."""
     if wl.preload_tokens:
@@ -93,7 +100,7 @@ def run_oracle_schedule(wl: Workload, n_updates: int, cfg_over=None, stream: int
         out = ho.oracle_step(st, K, V, Q)
         ids = np.concatenate([ids, np.broadcast_to(new_ids, (wl.n_layers, n))], axis=1)
         if out["evicted"]:
-            ids = np.take_along_axis(ids, out["kept"], axis=1)
+            ids = take_ids(ids, out["kept"])
         history.append(dict(out=out, ids=ids.copy(), V_pre=V_pre, V_new=V, K_new=K, Q=Q, pre_len=pre_len))
     return cfg, st, fd, ids, history
 

@@ -24,8 +24,9 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_config_struct_matches_header_size():
-    # 15 int32 + 3 float + int32 + 4 float + int32 + float + 3 int32 + 6 int32 = 34 x 4 bytes
-    assert C.sizeof(hb.HermesConfig) == 34 * 4
+    # 15 int32 + 3 float + int32 + 4 float + int32 + float + 3 int32 + 8 int32 = 36 x 4 bytes
+    assert C.sizeof(hb.HermesConfig) == 36 * 4
+    assert hb.hermes_default_config().reindex_mode == 0
     cfg = hb.hermes_default_config()
     assert (cfg.omega0, cfg.gamma) == (0.75, pytest.approx(0.6))
     assert (cfg.lambda_shallow, cfg.lambda_middle, cfg.lambda_deep) == (pytest.approx(0.1), pytest.approx(0.3), pytest.approx(0.4))
@@ -60,6 +61,14 @@ def test_invalid_configs_are_rejected(field, value):
 
 
 @pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU failure mode")
+def test_lazy_reindex_needs_room_below_max_position():
+    wl = CONFIGS["llava_ov_7b"]
+    bad = hb.config_for_workload(wl, reindex_mode=hb.HERMES_REINDEX_LAZY, max_position=wl.budget + wl.chunk_tokens)
+    assert hb.hermes_workspace_bytes(bad) == 0
+    ok = hb.config_for_workload(wl, reindex_mode=hb.HERMES_REINDEX_LAZY, max_position=32768)
+    assert hb.hermes_workspace_bytes(ok) > hb.hermes_workspace_bytes(hb.config_for_workload(wl))   # larger rotary table
+
+
 def test_create_without_gpu_fails_loudly():
     cfg = hb.config_for_workload(CONFIGS["toy"])
     with pytest.raises(hb.HermesError) as e:

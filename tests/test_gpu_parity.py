@@ -175,3 +175,29 @@ def test_determinism_and_host_api():
             assert torch.equal(a[l][key], b[l][key])          # same inputs -> same bits
             assert torch.equal(a[l][key], c[l][key])          # host-buffer entry point == device entry point
         assert torch.equal(kept[0, l].cuda(), a[l]["last_kept"])
+
+
+def test_lazy_reindexing_toy_and_bf16():
+    """DESIGN f2 (PAPER.md:126-128): lazy mode copies kept keys bit for bit and keeps their original indices;
+    the step after which the next chunk would cross max_position re-indexes exactly like the eager path."""
+    wl = CONFIGS["toy"]
+    ls, reps = _run(wl, 10, cfg_over=dict(reindex_mode=hb.HERMES_REINDEX_LAZY, max_position=300),
+                    oracle_over=dict(reindex_mode="lazy", max_position=300, max_chunk_span=wl.chunk_tokens))
+    fd = ls.feeders[0]
+    for l in range(wl.n_layers):                    # every key == RoPE(k0[id], its current position)
+        v = hb.hermes_get_cache(ls.h, 0, l)
+        pos = v["pos"].cpu().numpy().astype(np.int64)
+        k0 = np.stack([fd.k0_by_id[int(t)][l] for t in ls.ids[0][l]])[None]
+        ref = rope_at_arrival(k0, pos, wl)[0]
+        np.testing.assert_allclose(v["k"].float().cpu().numpy(), ref, atol=3e-5)
+        assert (np.diff(pos[0]) > 0).all() and pos.max() < 300
+    ls.close()
+    # bf16, multi-tile, tcgen05 scoring; max_position chosen so that the 4th checked update re-indexes
+    wl = CONFIGS["llava_ov_7b"].scaled(n_layers=6, budget=784, probe_tokens=16)
+    mp = 784 + 196 * 5
+    ls, reps = _run(wl, 6, cfg_over=dict(reindex_mode=hb.HERMES_REINDEX_LAZY, max_position=mp),
+                    oracle_over=dict(reindex_mode="lazy", max_position=mp, max_chunk_span=wl.chunk_tokens))
+    v = hb.hermes_get_cache(ls.h, 0, 0)
+    assert int(v["pos"].max()) < mp
+    assert sum(r["k_mismatch_bits"] for r in reps) == 0
+    ls.close()
