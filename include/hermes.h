@@ -81,6 +81,10 @@ typedef struct {
                                    re-indexes only at the step after which the next chunk (max_chunk_tokens
                                    positions; M-RoPE: its temporal steps) would exceed max_position        */
   int32_t max_position;         /* LAZY: the model's position limit (> pos_offset + budget + chunk span) */
+  int32_t summary_token;        /* 1: every deep layer keeps budget-1 tokens by Top-K and appends ONE summary
+                                   token of the evicted ones (Alg. 1) in slot budget-1 at
+                                   position pos_offset+budget-1; last_kept[budget-1] = -1 marks it.  Needs
+                                   HERMES_ROPE_1D and HERMES_REINDEX_EAGER                              */
   int32_t score_path;           /* HERMES_SCORE_*: AUTO picks tcgen05 when the contraction is dense */
   int32_t device;               /* CUDA device ordinal                                         */
 } hermes_config;
@@ -145,7 +149,7 @@ int hermes_device_status(hermes_t *h, int32_t *status_out);
  * hermes_get_profile() synchronises on the last call's events and writes up to n kernel durations in
  * milliseconds, in HERMES_K_* order (0 for kernels that did not run); returns the count written.      */
 enum { HERMES_K_APPEND = 0, HERMES_K_SCORE_STATS = 1, HERMES_K_SCORE_COMBINE = 2,
-       HERMES_K_SCORE_COLSUM = 3, HERMES_K_SELECT = 4, HERMES_K_GATHER = 5, HERMES_K_COUNT = 6 };
+       HERMES_K_SCORE_COLSUM = 3, HERMES_K_SELECT = 4, HERMES_K_GATHER = 5, HERMES_K_SUMMARY = 6, HERMES_K_COUNT = 7 };
 int hermes_set_profiling(hermes_t *h, int32_t enable);
 int hermes_get_profile(hermes_t *h, float *ms_out, int32_t n);
 

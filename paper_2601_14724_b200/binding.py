@@ -18,7 +18,7 @@ HERMES_ROPE_1D, HERMES_ROPE_M3D = 0, 1
 HERMES_REINDEX_EAGER, HERMES_REINDEX_LAZY = 0, 1
 HERMES_NORM_MAX, HERMES_NORM_SUM = 0, 1
 HERMES_SCORE_AUTO, HERMES_SCORE_SIMT, HERMES_SCORE_TCGEN05 = 0, 1, 2
-HERMES_K_NAMES = ("append", "score_stats", "score_combine", "score_colsum", "select", "gather")
+HERMES_K_NAMES = ("append", "score_stats", "score_combine", "score_colsum", "select", "gather", "summary")
 
 EXPORTS = ("hermes_default_config", "hermes_workspace_bytes", "hermes_create", "hermes_append_chunk",
            "hermes_append_chunk_host", "hermes_get_cache", "hermes_len", "hermes_device_status",
@@ -37,7 +37,7 @@ class HermesConfig(C.Structure):
                 ("rope_theta", C.c_float), ("mrope_section", C.c_int32 * 3),
                 ("mrope_compact_axes", C.c_int32), ("mrope_grid_h", C.c_int32),
                 ("mrope_grid_w", C.c_int32), ("pos_offset", C.c_int32), ("reindex_mode", C.c_int32),
-                ("max_position", C.c_int32), ("score_path", C.c_int32),
+                ("max_position", C.c_int32), ("summary_token", C.c_int32), ("score_path", C.c_int32),
                 ("device", C.c_int32)]
 
 

@@ -17,6 +17,9 @@ struct Geom {
   int n_axes;       // 1 (1D RoPE) or 3 (M-RoPE)
   int row_elems;    // Hkv * d elements per token row
   int n_shallow;    // layers [0, n_shallow) are pure recency (Eq. 1) and are not scored
+  int n_deep;       // layers [L - n_deep, L) are the deep stage
+  int summary;      // 1: deep layers keep budget-1 tokens and append one summary token (Alg. 1)
+  int n_evict_max;  // capacity of the evicted index lists: cap - budget + 1
   int p_max;        // max probe tokens (row capacity of the stat buffers = Hq * p_max)
   int pos_offset;
   int sec_t, sec_h; // M-RoPE: pairs [0,sec_t) -> t, [sec_t, sec_t+sec_h) -> h, rest -> w
@@ -35,6 +38,7 @@ struct Geom {
   float* scores;    // [B*L][cap]  smoothed scores S~ of the last eviction (a3)
   int32_t* kept;    // [B*L][budget] ascending kept indices I_l (a4)
   int32_t* delta;   // [B*L][n_axes][budget] p_new - p_old of every kept token (a6 -> a7)
+  int32_t* evicted; // [B*L][n_evict_max] ascending evicted indices (summary-token layers only)
   float2* rope_tab; // [table_rows][d/2] (cos, sin)(-r * theta_j) for r = row index
   double* rope_freq;// [d/2] theta_j in fp64 (slow path for deltas outside the table)
   float* omega;     // [L] weight of the recency term (Eq. 3-4); 1 shallow, 0 deep

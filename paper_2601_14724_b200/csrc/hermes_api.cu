@@ -7,6 +7,7 @@
 #include "k_gather.cuh"
 #include "k_score_simt.cuh"
 #include "k_select.cuh"
+#include "k_summary.cuh"
 #include "k_score_tc.cuh"
 
 using namespace hk;
@@ -88,7 +89,8 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   g.B = c->n_streams; g.L = c->n_layers; g.Hq = c->n_q_heads; g.Hkv = c->n_kv_heads;
   g.G = c->n_q_heads / c->n_kv_heads; g.d = c->head_dim;
   g.cap = y.cap; g.budget = c->budget; g.n_axes = y.n_axes; g.row_elems = c->n_kv_heads * c->head_dim;
-  g.n_shallow = y.n_shallow; g.p_max = c->max_probe_tokens; g.pos_offset = c->pos_offset;
+  g.n_shallow = y.n_shallow; g.n_deep = y.n_deep; g.summary = c->summary_token; g.n_evict_max = y.cap - c->budget + 1;
+  g.p_max = c->max_probe_tokens; g.pos_offset = c->pos_offset;
   g.sec_t = c->mrope_section[0]; g.sec_h = c->mrope_section[1];
   g.compact_axes = c->mrope_compact_axes; g.grid_h = c->mrope_grid_h; g.grid_w = c->mrope_grid_w;
   g.table_rows = y.table_rows; g.n_vh_max = y.n_vh_max;
@@ -101,6 +103,7 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   g.scores = reinterpret_cast<float*>(h->ws + y.scores);
   g.kept = reinterpret_cast<int32_t*>(h->ws + y.kept);
   g.delta = reinterpret_cast<int32_t*>(h->ws + y.delta);
+  g.evicted = reinterpret_cast<int32_t*>(h->ws + y.evicted);
   g.rope_tab = reinterpret_cast<float2*>(h->ws + y.rope_tab);
   g.rope_freq = reinterpret_cast<double*>(h->ws + y.rope_freq);
   g.omega = reinterpret_cast<float*>(h->ws + y.omega);
@@ -311,6 +314,12 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
       if (g.L > g.n_shallow)
         launch_pdl(k_wsum, dim3((Tn + 255) / 256, g.B * (g.L - g.n_shallow)), dim3(256), 0, s, g, Tn, n_probe, h->n_vh);
       launch_pdl(k_select, dim3(BL), dim3(kSelThreads), size_t(Tn) * 4, s, g, h->cur, Tn, c.forget_rate, int(c.norm_mode == HERMES_NORM_SUM), r_norm_sum, int(reindex));
+    }
+    if (c.summary_token && h->lay.n_deep > 0) {
+      Prof p(h, HERMES_K_SUMMARY, s);
+      const dim3 sgrid(g.Hkv, g.B * h->lay.n_deep), sblock(64 * kSumLanes);
+      if (c.dtype == HERMES_BF16) launch_pdl(k_summary<__nv_bfloat16>, sgrid, sblock, 0, s, g, h->cur, Tn);
+      else launch_pdl(k_summary<float>, sgrid, sblock, 0, s, g, h->cur, Tn);
     }
     {
       Prof p(h, HERMES_K_GATHER, s);

@@ -15,7 +15,7 @@ namespace hk {
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {           // byte offsets into the workspace
-  size_t kc, vc, posc, colsum, wsum, wmax, rowstat, partial, scores, kept, delta, rope_tab, rope_freq, omega, lambda,
+  size_t kc, vc, posc, colsum, wsum, wmax, rowstat, partial, scores, kept, delta, evicted, rope_tab, rope_freq, omega, lambda,
       status, seg_cnt, stage_k, stage_v, stage_q, tmaps, total;
   int cap, n_axes, n_part_max, table_rows, n_shallow, n_middle, n_deep, n_vh_max;
   size_t esize, row_bytes;
@@ -57,6 +57,9 @@ inline const char* validate(const hermes_config& c) {
   }
   if (c.pos_offset < 0) return "pos_offset must be >= 0";
   if (c.reindex_mode != HERMES_REINDEX_EAGER && c.reindex_mode != HERMES_REINDEX_LAZY) return "bad reindex_mode";
+  if (c.summary_token != 0 && c.summary_token != 1) return "summary_token must be 0 or 1";
+  if (c.summary_token && (c.rope_mode != HERMES_ROPE_1D || c.reindex_mode != HERMES_REINDEX_EAGER || c.budget < 2))
+    return "summary tokens need 1D RoPE, eager re-indexing and budget >= 2";
   if (c.reindex_mode == HERMES_REINDEX_LAZY) {
     const long long span = c.rope_mode == HERMES_ROPE_M3D
         ? (c.max_chunk_tokens + c.mrope_grid_h * c.mrope_grid_w - 1) / (c.mrope_grid_h * c.mrope_grid_w) : c.max_chunk_tokens;
@@ -84,7 +87,7 @@ inline Layout make_layout(const hermes_config& c) {
     const int tpt = c.mrope_grid_h * c.mrope_grid_w;
     y.table_rows = c.budget + (c.max_chunk_tokens + tpt - 1) / tpt + 2;
   } else {
-    y.table_rows = y.cap - c.budget + 1;
+    y.table_rows = y.cap - c.budget + 1 + (c.summary_token ? 1 : 0);   // summary layers evict one token more
   }
   // lazy mode: a re-index step moves positions from anywhere below the limit down to the compact range
   if (c.reindex_mode == HERMES_REINDEX_LAZY) y.table_rows = std::max(y.table_rows, c.max_position - c.pos_offset + 2);
@@ -103,6 +106,7 @@ inline Layout make_layout(const hermes_config& c) {
   y.scores = take(BL * y.cap * 4);
   y.kept = take(BL * c.budget * 4);
   y.delta = take(BL * y.n_axes * c.budget * 4);
+  y.evicted = take(BL * size_t(y.cap - c.budget + 1) * 4);
   y.rope_tab = take(size_t(y.table_rows) * (c.head_dim / 2) * 8);
   y.rope_freq = take(size_t(c.head_dim / 2) * 8);
   y.omega = take(size_t(c.n_layers) * 4);

@@ -105,7 +105,7 @@ k_gather(Geom g, int cur) {
   while (true) {
     const int u = idx - s * upr;
     const int e = (u / uph) * g.d + (u % uph) * V;
-    const size_t so = size_t(src) * g.row_elems + e;
+    const size_t so = size_t(max(src, 0)) * g.row_elems + e;   // src < 0: the summary-token slot, written by k_summary
     uint4 klo = ldg_stream(ks + so), khi = ldg_stream(ks + so + half);
     const uint4 vlo = ldg_stream(vs + so), vhi = ldg_stream(vs + so + half);
     // prefetch the next step's row index and deltas
@@ -122,8 +122,10 @@ k_gather(Geom g, int cur) {
     for (int a = 0; a < NAX; ++a) any |= dl[a] != 0;
     if (any) rotate_unit<T, NAX>(g, dl, (u % uph) * V, klo, khi);
     const size_t dof = size_t(s) * g.row_elems + e;
-    stg_stream(kd + dof, klo); stg_stream(kd + dof + half, khi);
-    stg_stream(vd + dof, vlo); stg_stream(vd + dof + half, vhi);
+    if (src >= 0) {
+      stg_stream(kd + dof, klo); stg_stream(kd + dof + half, khi);
+      stg_stream(vd + dof, vlo); stg_stream(vd + dof + half, vhi);
+    }
     if (!more) break;
     idx = idx_n; s = s_n; src = src_n;
 #pragma unroll

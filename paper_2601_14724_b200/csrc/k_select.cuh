@@ -176,7 +176,10 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
       }
     }
   }
-  if (tid == 0) { sel_prefix = 0u; sel_remaining = Tn - g.budget; }
+  // deep layers of a summary-token cache keep one token fewer: slot budget-1 is the summary token (DESIGN f1)
+  const bool summ = g.summary && l >= g.L - g.n_deep;
+  const int n_keep = g.budget - (summ ? 1 : 0);
+  if (tid == 0) { sel_prefix = 0u; sel_remaining = Tn - n_keep; }
   for (int i = tid; i < 32 * 256; i += kSelThreads) whist[i] = 0;
   __syncthreads();
 
@@ -289,6 +292,7 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
       const int lt_before = (pre & 0xFFFF) + __popc(lt & lane_lt);
       const int eq_before = (pre >> 16) + __popc(eq & lane_lt);
       const bool evict = key < vstar || (key == vstar && eq_before < r_eq);
+      if (summ && i < Tn && evict) g.evicted[size_t(bl) * g.n_evict_max + lt_before + min(eq_before, r_eq)] = i;
       if (i < Tn && !evict) {
         const int out = i - lt_before - min(eq_before, r_eq);            // slot of token i among the kept
         kept[out] = i;
@@ -304,6 +308,9 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
   SEL_T(5);
   if (blockIdx.x == 5 && threadIdx.x == 0) printf("select phases (cycles): setup %lld scores %lld radix %lld count+scan %lld write %lld\n", tstamp[1]-tstamp[0], tstamp[2]-tstamp[1], tstamp[3]-tstamp[2], tstamp[6]-tstamp[4], tstamp[5]-tstamp[6]);
 #endif
+  if (summ && tid == 0) {                               // the summary token's slot (filled by k_summary)
+    kept[n_keep] = -1; pos_new[n_keep] = g.pos_offset + n_keep; dl1[n_keep] = 0;
+  }
   if (g.n_axes == 1) return;
   __syncthreads();                                      // kept[] visible to the whole block
 

@@ -15,7 +15,7 @@ import numpy as np
 import torch
 
 import paper_2601_14724_b200 as hb
-from helpers import Feeder, bf16_ulp, fill_chunks, oracle_config
+from helpers import Feeder, bf16_ulp, fill_chunks, oracle_config, take_ids
 from oracle import hermes_oracle as ho
 
 SCORE_RTOL = 1e-3
@@ -94,7 +94,7 @@ class LockStep:
             for b in range(self.B):
                 kept = np.stack([hb.hermes_get_cache(self.h, b, l)["last_kept"].cpu().numpy()
                                  for l in range(self.wl.n_layers)]).astype(np.int64)
-                self.ids[b] = np.take_along_axis(self.ids[b], kept, axis=1)
+                self.ids[b] = take_ids(self.ids[b], kept)
 
     # ---- schedule -------------------------------------------------------------------------------
     def fill(self):
@@ -139,6 +139,7 @@ class LockStep:
         rep = dict(stream=b, T=out["T"], band_layers=0, band_tokens=0, max_score_rel=0.0, k_mismatch_bits=0,
                    k_max_err_norm=0.0)
         for l in range(wl.n_layers):
+            M = wl.budget
             v = hb.hermes_get_cache(self.h, b, l)
             assert v["len"] == M and v["last_T"] == out["T"]
             s_gpu = v["last_scores"].cpu().numpy().astype(np.float64)
@@ -149,6 +150,18 @@ class LockStep:
             rep["max_score_rel"] = max(rep["max_score_rel"], float(rel.max()))
             kept_gpu = v["last_kept"].cpu().numpy().astype(np.int64)
             kept_or = out["kept"][l]
+            k_gpu = v["k"].float().cpu().numpy(); v_gpu = v["v"].float().cpu().numpy()
+            p_gpu = v["pos"].cpu().numpy().astype(np.int64)
+            if kept_or[-1] < 0:
+                # summary token (DESIGN f1) in the last slot: computed values, so K AND V get the K tolerance
+                assert kept_gpu[-1] == -1 and p_gpu[0, -1] == st.pos[l, 0, M - 1]
+                for g_, o_ in ((k_gpu[-1], st.K[l, M - 1]), (v_gpu[-1], st.V[l, M - 1])):
+                    tol = np.maximum(K_RTOL * np.abs(o_), 2 * bf16_ulp(o_) if wl.dtype == "bf16" else 0.0) + 1e-30
+                    assert (np.abs(g_.astype(np.float64) - o_) <= tol).all(), f"layer {l}: summary token off"
+                rep["summary_layers"] = rep.get("summary_layers", 0) + 1
+                kept_gpu, kept_or = kept_gpu[:-1], kept_or[:-1]
+                k_gpu, v_gpu, p_gpu = k_gpu[:-1], v_gpu[:-1], p_gpu[:, :-1]
+                M = M - 1
             assert len(kept_gpu) == M and (np.diff(kept_gpu) > 0).all() and kept_gpu[0] >= 0 and kept_gpu[-1] < out["T"]
             same = np.array_equal(kept_gpu, kept_or)
             if not same:
@@ -159,8 +172,6 @@ class LockStep:
                 rep["band_layers"] += 1
                 rep["band_tokens"] += len(diff)
             # rows both sides kept: V bit-exact, K within tolerance, positions exact when the sets agree
-            k_gpu = v["k"].float().cpu().numpy(); v_gpu = v["v"].float().cpu().numpy()
-            p_gpu = v["pos"].cpu().numpy().astype(np.int64)
             if same:
                 sel_g = sel_o = np.arange(M)
                 assert np.array_equal(p_gpu, st.pos[l, :, :M]), f"layer {l}: positions differ"

@@ -201,3 +201,16 @@ def test_lazy_reindexing_toy_and_bf16():
     assert int(v["pos"].max()) < mp
     assert sum(r["k_mismatch_bits"] for r in reps) == 0
     ls.close()
+
+
+def test_summary_token_toy_and_bf16():
+    """DESIGN f1 (Alg. 1): deep layers keep |M| - 1 tokens and append the summary of the evicted ones."""
+    wl = CONFIGS["toy"]
+    ls, reps = _run(wl, 6, cfg_over=dict(summary_token=1), oracle_over=dict(summary_token=True))
+    assert all(r.get("summary_layers") == 1 for r in reps)                     # 4 layers: one deep
+    assert (ls.ids[0][3] == -1).sum() >= 1 and (ls.ids[0][:3] >= 0).all()
+    ls.close()
+    wl = CONFIGS["llava_ov_7b"].scaled(n_layers=7, budget=784, probe_tokens=16)    # 1 shallow, 4 middle, 2 deep
+    ls, reps = _run(wl, 3, n_warm=1, cfg_over=dict(summary_token=1), oracle_over=dict(summary_token=True))
+    assert all(r.get("summary_layers") == 2 for r in reps)
+    ls.close()
