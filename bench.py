@@ -147,7 +147,12 @@ def run_ours(args):
     wl = workload_by_name(args.workload)
     B = wl.n_streams
     tdt = torch.bfloat16 if wl.dtype == "bf16" else torch.float32
-    cfg = hb.config_for_workload(wl, device=local_rank, score_path={"auto": 0, "simt": 1, "tcgen05": 2}[args.score_path])
+    over = dict(score_path={"auto": 0, "simt": 1, "tcgen05": 2}[args.score_path])
+    if args.reindex == "lazy":                               # the paper's default for streaming
+        over.update(reindex_mode=hb.HERMES_REINDEX_LAZY, max_position=args.max_position)
+    if args.summary_token:
+        over.update(summary_token=1)
+    cfg = hb.config_for_workload(wl, device=local_rank, **over)
     h = hb.hermes_create(cfg)
 
     host_pool = [tuple(torch.from_numpy(x).to(tdt).pin_memory() for x in s) for s in make_pool(wl, rank, POOL)]
@@ -266,7 +271,7 @@ def run_ours(args):
                    "l2": (f"cache slabs touched per step: {ws_mb:.0f} MB read + {wr_mb:.0f} MB written "
                           + ("(exceeds the 126 MB L2)" if ws_mb + wr_mb > 252 else "(comparable to the 126 MB L2: no flush, L2-assisted)")
                           + f"; inputs cycle through {POOL} chunk/probe sets"),
-                   "score_path": score_path},
+                   "score_path": score_path, "reindex": args.reindex, "summary_token": bool(args.summary_token)},
         "e2e": {"value": job_value(wl, world, B, ms_e2e), "unit": UNIT, "ms_per_step": ms_e2e,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e},
         "gpu_launches": launches,
@@ -335,6 +340,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="llava_ov_7b", help="one of %s, or sweep:<budget>:<probe>" % sorted(CONFIGS))
     ap.add_argument("--score-path", default="auto", choices=["auto", "simt", "tcgen05"])
+    ap.add_argument("--reindex", default="eager", choices=["eager", "lazy"])
+    ap.add_argument("--max-position", type=int, default=32768, help="lazy re-indexing: the model's position limit")
+    ap.add_argument("--summary-token", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

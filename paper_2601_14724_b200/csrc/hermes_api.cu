@@ -106,6 +106,8 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   g.evicted = reinterpret_cast<int32_t*>(h->ws + y.evicted);
   g.rope_tab = reinterpret_cast<float2*>(h->ws + y.rope_tab);
   g.rope_freq = reinterpret_cast<double*>(h->ws + y.rope_freq);
+  g.sum_tab = reinterpret_cast<float2*>(h->ws + y.sum_tab);
+  g.sum_tab_zero = y.cap - c->budget + 1;        // deltas of the summary alignment lie in [-(cap - budget + 1), budget)
   g.omega = reinterpret_cast<float*>(h->ws + y.omega);
   g.lambda = reinterpret_cast<float*>(h->ws + y.lambda);
   g.status = reinterpret_cast<int32_t*>(h->ws + y.status);
@@ -137,6 +139,15 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   auto up = [&](void* dst, const void* src, size_t n) { if (e == cudaSuccess) e = cudaMemcpy(dst, src, n, cudaMemcpyHostToDevice); };
   up(g.omega, omega.data(), L * 4); up(g.lambda, lambda.data(), L * 4);
   up(g.rope_freq, freq.data(), half * 8); up(g.rope_tab, tab.data(), tab.size() * 8);
+  if (c->summary_token) {                          // (cos, sin)(delta * theta_j) for every delta Alg. 1 can meet
+    std::vector<float2> st(size_t(y.cap + 2) * half);
+    for (int r = 0; r < y.cap + 2; ++r)
+      for (int j = 0; j < half; ++j) {
+        const double ang = double(r - g.sum_tab_zero) * freq[j];
+        st[size_t(r) * half + j] = make_float2(float(std::cos(ang)), float(std::sin(ang)));
+      }
+    up(g.sum_tab, st.data(), st.size() * 8);
+  }
   if (e == cudaSuccess) e = cudaMemset(g.status, 0, 256);
   if (e == cudaSuccess) e = cudaMemset(h->ws + y.seg_cnt, 0, size_t(g.B) * L * y.n_vh_max * 4);
   if (e == cudaSuccess) e = cudaMemset(g.posc, 0, size_t(g.B) * L * 2 * y.n_axes * y.cap * 4);
@@ -318,8 +329,9 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
     if (c.summary_token && h->lay.n_deep > 0) {
       Prof p(h, HERMES_K_SUMMARY, s);
       const dim3 sgrid(g.Hkv, g.B * h->lay.n_deep), sblock(64 * kSumLanes);
-      if (c.dtype == HERMES_BF16) launch_pdl(k_summary<__nv_bfloat16>, sgrid, sblock, 0, s, g, h->cur, Tn);
-      else launch_pdl(k_summary<float>, sgrid, sblock, 0, s, g, h->cur, Tn);
+      const size_t ssm = size_t(Tn - c.budget + 1) * 8;
+      if (c.dtype == HERMES_BF16) launch_pdl(k_summary<__nv_bfloat16>, sgrid, sblock, ssm, s, g, h->cur, Tn);
+      else launch_pdl(k_summary<float>, sgrid, sblock, ssm, s, g, h->cur, Tn);
     }
     {
       Prof p(h, HERMES_K_GATHER, s);

@@ -15,7 +15,7 @@ namespace hk {
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {           // byte offsets into the workspace
-  size_t kc, vc, posc, colsum, wsum, wmax, rowstat, partial, scores, kept, delta, evicted, rope_tab, rope_freq, omega, lambda,
+  size_t kc, vc, posc, colsum, wsum, wmax, rowstat, partial, scores, kept, delta, evicted, rope_tab, rope_freq, sum_tab, omega, lambda,
       status, seg_cnt, stage_k, stage_v, stage_q, tmaps, total;
   int cap, n_axes, n_part_max, table_rows, n_shallow, n_middle, n_deep, n_vh_max;
   size_t esize, row_bytes;
@@ -109,6 +109,7 @@ inline Layout make_layout(const hermes_config& c) {
   y.evicted = take(BL * size_t(y.cap - c.budget + 1) * 4);
   y.rope_tab = take(size_t(y.table_rows) * (c.head_dim / 2) * 8);
   y.rope_freq = take(size_t(c.head_dim / 2) * 8);
+  y.sum_tab = take(c.summary_token ? size_t(y.cap + 2) * (c.head_dim / 2) * 8 : 0);
   y.omega = take(size_t(c.n_layers) * 4);
   y.lambda = take(size_t(c.n_layers) * 4);
   y.status = take(256);

@@ -2,20 +2,21 @@
 //   v_sum = Mean(V_p);  k_sum = Mean(ApplyDelta(K_p, RotaryDelta(P_p -> t))),  t = pos_offset + budget - 1,
 // written to slot budget-1 of the NEW buffer (k_gather leaves that slot alone; k_select set its position).
 // One block per (KV head, stream x deep layer): thread = (rotary pair j, token lane q); token lane q walks the
-// evicted tokens q, q + kSumLanes, ...  Angles in fp64 (deltas reach +-budget, far outside the eager rotary
-// table), cos / sin and the rotation in fp32 without FMA exactly as in k_gather, sums in fp64, lanes reduced
+// evicted tokens q, q + kSumLanes, ...  (cos, sin) from a table built in fp64 at create time for every delta in
+// [-(cap - budget + 1), budget) (fp64 sincos otherwise), rotation in fp32 without FMA exactly as in k_gather, sums in fp64, lanes reduced
 // in shared memory in fixed order, one rounding to the storage dtype.  ~E x 2 KB per layer: latency only.
 #pragma once
 #include "common.cuh"
 
 namespace hk {
 
-constexpr int kSumLanes = 8;
+constexpr int kSumLanes = 16;
 
 template <typename T>
 __global__ void __launch_bounds__(64 * kSumLanes)
 k_summary(Geom g, int cur, int Tn) {
   __shared__ double red[kSumLanes][4][64];                 // [token lane][kx, ky, vx, vy][pair]
+  extern __shared__ int s_list[];                          // [2][n_ev]: source row, rotary delta of every evicted token
   pdl_wait();
   pdl_launch_dependents();
   const int half = g.d >> 1;
@@ -30,16 +31,25 @@ k_summary(Geom g, int cur, int Tn) {
   const T* vs = reinterpret_cast<const T*>(g.vc) + slab_src * g.cap * g.row_elems + kvh * g.d;
   const int32_t* pos_old = g.posc + slab_src * g.cap;      // 1D RoPE only (validated at create)
   const int32_t* ev = g.evicted + size_t(bl) * g.n_evict_max;
+  int* s_src = s_list;
+  int* s_dl = s_list + n_ev;
+  for (int i = threadIdx.x; i < n_ev; i += blockDim.x) {   // one dependent-load chain per token, all in flight at once
+    const int src = __ldcg(ev + i);
+    s_src[i] = src; s_dl[i] = t - __ldcg(pos_old + src);
+  }
+  __syncthreads();
   for (int j0 = 0; j0 < half; j0 += 64) {
     const int jj = j0 + j;
     double kx = 0.0, ky = 0.0, vx = 0.0, vy = 0.0;
     if (jj < half) {
-      const double theta = g.rope_freq[jj];
+#pragma unroll 4
       for (int i = q; i < n_ev; i += kSumLanes) {
-        const int src = __ldcg(ev + i);
-        const int delta = t - __ldcg(pos_old + src);
-        const double ang = double(delta) * theta;
-        const float c = float(cos(ang)), s = float(sin(ang));
+        const int src = s_src[i];
+        const int delta = s_dl[i];
+        const int r = delta + g.sum_tab_zero;
+        float c, s;
+        if (r >= 0 && r < g.cap + 2) { const float2 cs = __ldg(g.sum_tab + size_t(r) * half + jj); c = cs.x; s = cs.y; }
+        else { const double ang = double(delta) * g.rope_freq[jj]; c = float(cos(ang)); s = float(sin(ang)); }   // explicit pos_start jumps
         const size_t o = size_t(src) * g.row_elems;
         const float x = Elem<T>::to_float(__ldcg(ks + o + jj)), y = Elem<T>::to_float(__ldcg(ks + o + jj + half));
         float xr = x, yr = y;
