@@ -22,6 +22,10 @@ Parity status: every function below is pinned by
 PARITY UNPINNED (the paper prints no number that depends on them): the choice
 of normalisation factor alpha (DESIGN c2), the value of the forgetting rate k
 (c1), the mean over heads / probe rows (c3) and the softmax domain (c4).
+Also unpinned against the authors' code: where the summary token sits, its target
+position and the budget accounting (DESIGN f1), and the exact lazy re-index trigger
+(DESIGN f2); the arithmetic of both IS pinned (tests/test_oracle_summary.py,
+tests/test_oracle_lazy.py).
 
 Storage convention: K and V are held as float32 arrays whose values are exactly
 representable in the storage dtype ("f32" or "bf16"); positions are int64.
