@@ -81,11 +81,12 @@ struct TcSmem {
   uint8_t* k;        // K ring: [stage][2 halves][128 tokens][128 B]
   float* c;          // [512] per-row c_r (pass 2)
   float4* xch;       // [2][8][32] pass-1 exchange between the two token-half warps of a row block quarter
+  float2* xch2;      // [2][2][32] pass-1 exchange between the even- / odd-tile lane quarters of a half-full row block
   uint64_t* bars;    // mbarriers
   uint32_t* tmem;    // TMEM base address written by tcgen05.alloc
 };
 __host__ __device__ inline int tc_smem_bytes(int q_half_bytes, int n_kst) {
-  return 1024 + 2 * q_half_bytes + n_kst * kTcKStage + kTcRowsMax * 4 + 8192 + 256 + 16;
+  return 1024 + 2 * q_half_bytes + n_kst * kTcKStage + kTcRowsMax * 4 + 8192 + 1024 + 256 + 16;
 }
 __device__ inline TcSmem tc_carve(uint8_t* raw, const TcArgs& a) {
   uint8_t* p = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(raw) + 1023) & ~uintptr_t(1023));
@@ -94,6 +95,7 @@ __device__ inline TcSmem tc_carve(uint8_t* raw, const TcArgs& a) {
   s.k = p; p += a.n_kst * kTcKStage;
   s.c = reinterpret_cast<float*>(p); p += kTcRowsMax * 4;
   s.xch = reinterpret_cast<float4*>(p); p += 8192;
+  s.xch2 = reinterpret_cast<float2*>(p); p += 1024;
   s.bars = reinterpret_cast<uint64_t*>(p); p += 256;
   s.tmem = reinterpret_cast<uint32_t*>(p);
   return s;
@@ -197,6 +199,7 @@ __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const
     TcCursor g; g.init(a, s0 / a.spg);
     for (int u = s0; u < s1; ++u) {
       const int n_rb = (g.rs_valid(a) + 127) >> 7;
+      const bool shift = g.rs_valid(a) > 384 && g.rs_valid(a) <= 448;
       if (new_group) { ptx::mbar_wait(b.q_full, n_q & 1); ++n_q; new_group = false; }
       const bool last_seg_of_group = (u + 1 == s1) || x + 1 == a.spg;
       const int t_end = min(a.tpg, (x + 1) * kTcSegTiles);
@@ -210,6 +213,10 @@ __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const
           if (lane == 0) TC_TRACE(1, 2);
           const uint32_t qa_lo = q_lo + uint32_t(2 * hg) * 1024u, d0 = tmem_base + as * 256;
           const bool two = 2 * hg + 1 < n_rb;
+          // a fourth row block that is at most half full alternates between the lower (even tiles) and the
+          // upper (odd tiles) 64 TMEM lanes -- the A tile then starts 64 rows earlier -- so that all four SM
+          // sub-partitions carry the same exp2 load (see the epilogue)
+          const uint32_t sh = (shift && hg == 1 && (t & 1)) ? 512u : 0u;
           if (ptx::elect_one()) {
 #pragma unroll
             for (int kk = 0; kk < 8; ++kk)
@@ -218,7 +225,7 @@ __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const
             if (two) {
 #pragma unroll
               for (int kk = 0; kk < 8; ++kk)
-                ptx::mma_bf16_lohi(d0 + kTcTile, qa_lo + 1024u + (kk >> 2) * q_half16 + (kk & 3) * 2,
+                ptx::mma_bf16_lohi(d0 + kTcTile, qa_lo + 1024u - sh + (kk >> 2) * q_half16 + (kk & 3) * 2,
                                    kb_lo + (kk >> 2) * 1024u + (kk & 3) * 2, ptx::kSmemDescHiSw128, idesc, kk > 0);
             }
             ptx::mma_commit(&b.t_full[as]);
@@ -290,13 +297,16 @@ __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const
       const int rs_valid = g.rs_valid(a);
       const bool two = rs_valid > 256;                                   // the group has a second half-group
       const bool act0 = rbl * 128 + lg * 32 < rs_valid, act1 = (2 + rbl) * 128 + lg * 32 < rs_valid;
+      // half-full fourth row block: lanes 0-63 hold it on even tiles, lanes 64-127 on odd tiles (see the MMA warp)
+      const bool shift = rs_valid > 384 && rs_valid <= 448 && rbl == 1;
+      const bool act1_odd = lg >= 2 && 384 + (lg - 2) * 32 < rs_valid;
       const int t_end = min(a.tpg, (x + 1) * kTcSegTiles);
       for (int t = x * kTcSegTiles; t < t_end; ++t) {
         const int n_valid = a.Tn - (t * kTcTile + th * 64);
 #pragma unroll
         for (int hg = 0; hg < 2; ++hg) {
           if (hg == 1 && !two) break;
-          const bool act = (hg == 0 ? act0 : act1) && n_valid > 0;
+          const bool act = (hg == 0 ? act0 : (shift && (t & 1)) ? act1_odd : act1) && n_valid > 0;
           ptx::mbar_wait(&b.t_full[as], aph);
           ptx::tc_fence_after();
           if (tr) TC_TRACE(trole, 1);
@@ -324,13 +334,26 @@ __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const
         if (th == 0) {
           const float4 o = *xch;
           const float ma = fmaxf(m0, o.x), mb = fmaxf(m1, o.z);            // this half always saw a token: finite
-          const float za = z0 * fast_exp2(m0 - ma) + o.y * fast_exp2(o.x - ma);
-          const float zb = z1 * fast_exp2(m1 - mb) + o.w * fast_exp2(o.z - mb);
+          // a row / half that saw no token is (-inf, 0): keep it that way instead of exp2(-inf + inf)
+          const float za = ma == -INFINITY ? 0.f : z0 * fast_exp2(m0 - ma) + o.y * fast_exp2(o.x - ma);
+          const float zb = mb == -INFINITY ? 0.f : z1 * fast_exp2(m1 - mb) + o.w * fast_exp2(o.z - mb);
           float2* part = reinterpret_cast<float2*>(a.g.partial) +
                          (size_t(g.bl(a)) * a.spg + x) * (a.g.Hq * a.g.p_max) + g.stat_row0(a);
           const int row_a = rbl * 128 + lg * 32 + lane, row_b = row_a + 256;
           if (row_a < rs_valid) part[row_a] = make_float2(ma, za);
-          if (row_b < rs_valid) part[row_b] = make_float2(mb, zb);
+          if (!shift) {
+            if (row_b < rs_valid) part[row_b] = make_float2(mb, zb);
+          } else {
+            // the odd-tile share of rows 384 + (lg - 2) * 32 + lane sits in lane quarter lg >= 2: hand it to quarter lg - 2
+            float2* x2 = s.xch2 + ((u & 1) * 2 + (lg & 1)) * 32 + lane;
+            if (lg >= 2) *x2 = make_float2(mb, zb);
+            ptx::named_bar_sync(10 + (lg & 1), 64);
+            if (lg < 2 && row_b < rs_valid) {
+              const float2 o = *x2;
+              const float m = fmaxf(mb, o.x);                            // a segment holds at least one tile: not both -inf
+              part[row_b] = make_float2(m, zb * fast_exp2(mb - m) + o.y * fast_exp2(o.x - m));
+            }
+          }
         }
         m0 = m1 = -INFINITY; z0 = z1 = 0.f;
       }
