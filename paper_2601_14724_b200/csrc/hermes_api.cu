@@ -338,8 +338,9 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
       const int V = c.dtype == HERMES_BF16 ? 8 : 4;
       const int upr = g.Hkv * (g.d / 2 / V);
       const int total = g.budget * upr;
-      // ~4 resident blocks per SM over all slabs; every thread walks total / (gx * 256) units
-      const int want = std::max(1, (h->n_sm * 4 * 2 + BL - 1) / BL);
+      // 4 resident blocks per SM; 8 whole waves over all slabs measured best (118 -> 114 us at configs[1]; a
+      // partial extra wave, as the old rounding produced, cost 5 us): short blocks even out the per-SM HBM rates
+      const int want = std::max(1, (h->n_sm * 4 * 8) / BL);
       const int gx = std::max(1, std::min(want, (total + kGatherThreads - 1) / kGatherThreads));
       const dim3 grid(gx, BL);
       if (c.dtype == HERMES_BF16) {
