@@ -27,8 +27,8 @@ from workloads import CONFIGS, chunk_kv, probe_q, sweep_point  # noqa: E402
 METRIC, UNIT = "kv_tokens_managed_per_s", "tokens/s"
 POOL = 16          # distinct pre-generated chunk/probe sets cycled through the timed region
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at configs[1], transcribed from the one
-# `ncu --set full` capture summarised in profiles/r1b_ncu_full_summary.txt (command in profiles/r1b_README.md)
-NCU_TRAFFIC_BYTES = {"gather": 361.28e6 + 311.93e6, "score": 184.26e6 + 7.40e6 + 200.97e6 + 9.88e6,
+# `ncu --set full` capture summarised in profiles/r1c_ncu_full_summary.txt (command in profiles/r1c_README.md)
+NCU_TRAFFIC_BYTES = {"gather": 361.18e6 + 309.93e6, "score": 367.49e6 + 15.54e6,
                      "select": 1.44e6, "append": 11.25e6}
 
 
