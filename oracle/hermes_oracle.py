@@ -78,6 +78,7 @@ class OracleConfig:
     reindex_mode: str = "eager"       # "eager" | "lazy" (DESIGN f2)
     max_position: int = 0             # lazy: the model's position limit that triggers a re-index
     max_chunk_span: int = 0           # lazy: largest position span of one arriving chunk (tokens; M-RoPE: t steps)
+    probe_deep_begin: int = 0         # deep layers use probe rows [begin, P): the global prompt only (DESIGN f3)
     summary_token: bool = False       # deep layers: evicted tokens -> one summary token (Alg. 1; DESIGN f1)
     capacity: int = 0                 # slots per layer; 0 -> budget + largest chunk seen
 
@@ -417,7 +418,10 @@ def oracle_step(st: OracleStream, K_new: np.ndarray, V_new: np.ndarray,
     W = np.zeros((L, T), np.float64)
     for l in range(L):
         if layer_stage(cfg, l) != "shallow":
-            W[l] = attention_weights(Q_probe[l], st.K[l, :T], cfg.group, scale)
+            # hybrid guidance (App. B): the probe rows are [local prompt | global prompt]; middle
+            # layers use all of them, deep layers only the global part (DESIGN f3)
+            pb = cfg.probe_deep_begin if layer_stage(cfg, l) == "deep" else 0
+            W[l] = attention_weights(Q_probe[l][:, pb:], st.K[l, :T], cfg.group, scale)
 
     # 3-4. normalise, recency, layer weighting (Eq. 1-4); 5. smoothing (Eq. 5)
     S = raw_scores(cfg, W, T)
