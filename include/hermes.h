@@ -81,6 +81,9 @@ typedef struct {
                                    re-indexes only at the step after which the next chunk (max_chunk_tokens
                                    positions; M-RoPE: its temporal steps) would exceed max_position        */
   int32_t max_position;         /* LAZY: the model's position limit (> pos_offset + budget + chunk span) */
+  int32_t probe_deep_begin;     /* deep layers score with probe rows [begin, n_probe) only: Q_probe rows are
+                                   [local prompt | global prompt], middle layers use all (App. B);
+                                   0 = all rows everywhere                                              */
   int32_t summary_token;        /* 1: every deep layer keeps budget-1 tokens by Top-K and appends ONE summary
                                    token of the evicted ones (Alg. 1) in slot budget-1 at
                                    position pos_offset+budget-1; last_kept[budget-1] = -1 marks it.  Needs

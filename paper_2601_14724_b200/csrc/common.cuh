@@ -18,6 +18,7 @@ struct Geom {
   int row_elems;    // Hkv * d elements per token row
   int n_shallow;    // layers [0, n_shallow) are pure recency (Eq. 1) and are not scored
   int n_deep;       // layers [L - n_deep, L) are the deep stage
+  int probe_deep_begin; // deep layers use probe rows [begin, P) only (hybrid guidance, DESIGN f3)
   int summary;      // 1: deep layers keep budget-1 tokens and append one summary token (Alg. 1)
   int n_evict_max;  // capacity of the evicted index lists: cap - budget + 1
   int p_max;        // max probe tokens (row capacity of the stat buffers = Hq * p_max)

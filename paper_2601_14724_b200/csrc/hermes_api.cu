@@ -89,7 +89,7 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   g.B = c->n_streams; g.L = c->n_layers; g.Hq = c->n_q_heads; g.Hkv = c->n_kv_heads;
   g.G = c->n_q_heads / c->n_kv_heads; g.d = c->head_dim;
   g.cap = y.cap; g.budget = c->budget; g.n_axes = y.n_axes; g.row_elems = c->n_kv_heads * c->head_dim;
-  g.n_shallow = y.n_shallow; g.n_deep = y.n_deep; g.summary = c->summary_token; g.n_evict_max = y.cap - c->budget + 1;
+  g.n_shallow = y.n_shallow; g.n_deep = y.n_deep; g.summary = c->summary_token; g.probe_deep_begin = c->probe_deep_begin; g.n_evict_max = y.cap - c->budget + 1;
   g.p_max = c->max_probe_tokens; g.pos_offset = c->pos_offset;
   g.sec_t = c->mrope_section[0]; g.sec_h = c->mrope_section[1];
   g.compact_axes = c->mrope_compact_axes; g.grid_h = c->mrope_grid_h; g.grid_w = c->mrope_grid_w;
@@ -265,6 +265,7 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
   if (!K_new || !V_new) return fail(h, HERMES_EINVAL, "K_new / V_new must not be NULL");
   if (n_new <= 0) return fail(h, HERMES_EINVAL, "n_new = %d must be positive", n_new);
   if (Q_probe && (n_probe <= 0 || n_probe > c.max_probe_tokens)) return fail(h, HERMES_EINVAL, "n_probe = %d not in [1, %d]", n_probe, c.max_probe_tokens);
+  if (Q_probe && c.probe_deep_begin >= n_probe) return fail(h, HERMES_EINVAL, "probe_deep_begin %d leaves no probe row of %d for the deep layers", c.probe_deep_begin, n_probe);
   const int Tn = h->len + n_new;
   if (Tn > g.cap) return fail(h, HERMES_ECAPACITY, "len %d + n_new %d exceeds max_tokens %d", h->len, n_new, g.cap);
   // arrival positions (DESIGN c16): host-computable, strictly above every cached position

@@ -57,6 +57,7 @@ inline const char* validate(const hermes_config& c) {
   }
   if (c.pos_offset < 0) return "pos_offset must be >= 0";
   if (c.reindex_mode != HERMES_REINDEX_EAGER && c.reindex_mode != HERMES_REINDEX_LAZY) return "bad reindex_mode";
+  if (c.probe_deep_begin < 0 || c.probe_deep_begin >= c.max_probe_tokens) return "probe_deep_begin must lie in [0, max_probe_tokens)";
   if (c.summary_token != 0 && c.summary_token != 1) return "summary_token must be 0 or 1";
   if (c.summary_token && (c.rope_mode != HERMES_ROPE_1D || c.reindex_mode != HERMES_REINDEX_EAGER || c.budget < 2))
     return "summary tokens need 1D RoPE, eager re-indexing and budget >= 2";

@@ -57,7 +57,8 @@ k_score_simt(Geom g, const T* __restrict__ q_probe, int cur, int Tn, int P, floa
       q_s[rr][c] = (r0 + rr < R) ? Elem<T>::to_float(qg[size_t(r0 + rr) * D + c]) : 0.f;
     }
     if (kColsum && tid < kSimtRowChunk) {
-      const bool ok = r0 + tid < R;
+      // deep layers ignore the local-prompt rows (probe index < probe_deep_begin) of every query head
+      const bool ok = r0 + tid < R && !(l >= g.L - g.n_deep && (r0 + tid) % P < g.probe_deep_begin);
       stat_s[tid][0] = ok ? rowstat[(r0 + tid) * 2] : 0.f;
       stat_s[tid][1] = ok ? rowstat[(r0 + tid) * 2 + 1] : 0.f;   // 1/Z = 0 masks rows past R
     }

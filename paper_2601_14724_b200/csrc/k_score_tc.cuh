@@ -368,10 +368,12 @@ __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const
 // Pass-2 group prologue: merges each probe row's per-(segment, half) (m, z) partials of pass 1 in slot
 // order into c_r = m_r + log2 Z_r (shared memory); rows past the group get +inf: exp2(-inf) = 0.
 // 16 independent loads in flight per thread.  Kept out of line so its registers do not weigh on the hot loop.
-__device__ __noinline__ void tc_merge_rows(const float2* pr, int n_slot, int rows_total, int rs_valid, float* c_out, int et) {
+__device__ __noinline__ void tc_merge_rows(const float2* pr, int n_slot, int rows_total, int rs_valid, float* c_out, int et,
+                                           int row0, int P, int skip_below) {
   for (int i = et; i < kTcRowsMax; i += kTcEpiWarps * 32) {
     float c = INFINITY;
-    if (i < rs_valid) {
+    // skip_below > 0 (deep layers, DESIGN f3): probe rows below it (row = query head * P + probe index) are left out
+    if (i < rs_valid && (row0 + i) % P >= skip_below) {
       const float2* p2 = pr + i;
       float m = -INFINITY, zz = 0.f;
       for (int j0 = 0; j0 < n_slot; j0 += 16) {
@@ -507,7 +509,8 @@ __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const
         if (tr) TC_TRACE(trole, 5);
         const int bl = g.bl(a), rows_total = a.g.Hq * a.g.p_max;
         tc_merge_rows(reinterpret_cast<const float2*>(a.g.partial) + size_t(bl) * a.spg * rows_total + g.stat_row0(a),
-                      a.spg, rows_total, g.rs_valid(a), s.c, threadIdx.x - 64);
+                      a.spg, rows_total, g.rs_valid(a), s.c, threadIdx.x - 64, g.sc * a.RS, a.P,
+                      g.ls >= a.g.L - a.g.n_shallow - a.g.n_deep ? a.g.probe_deep_begin : 0);
         ptx::named_bar_sync(1, kTcEpiWarps * 32);
         if (tr) TC_TRACE(trole, 6);
         rs32 = (g.rs_valid(a) + 31) & ~31;

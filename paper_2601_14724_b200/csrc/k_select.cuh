@@ -93,7 +93,9 @@ k_wsum(Geom g, int Tn, int P, int n_vh) {
   if (i < Tn) {
     const float* c = g.colsum + size_t(bl) * g.n_vh_max * g.cap + i;
     for (int h = 0; h < n_vh; ++h) w += __ldcg(c + size_t(h) * g.cap);
-    w *= 1.0f / float(g.Hq * P);
+    const int l = bl % g.L;
+    const int p_eff = l >= g.L - g.n_deep ? P - g.probe_deep_begin : P;    // deep layers: global-prompt rows only
+    w *= 1.0f / float(g.Hq * p_eff);
     g.wsum[size_t(bl) * g.cap + i] = w;
   }
   const float m = warp_max(w);

@@ -214,3 +214,14 @@ def test_summary_token_toy_and_bf16():
     ls, reps = _run(wl, 3, n_warm=1, cfg_over=dict(summary_token=1), oracle_over=dict(summary_token=True))
     assert all(r.get("summary_layers") == 2 for r in reps)
     ls.close()
+
+
+def test_probe_row_ranges_simt_and_tcgen05():
+    """DESIGN f3 (App. B): deep layers score with the global-prompt rows [probe_deep_begin, P) only."""
+    ls, _ = _run(CONFIGS["toy"], 3, cfg_over=dict(probe_deep_begin=3), oracle_over=dict(probe_deep_begin=3))
+    assert hb.hermes_last_score_path(ls.h) == hb.HERMES_SCORE_SIMT
+    ls.close()
+    wl = CONFIGS["llava_ov_7b"].scaled(n_layers=7, budget=784, probe_tokens=24)
+    ls, _ = _run(wl, 2, n_warm=1, cfg_over=dict(probe_deep_begin=8), oracle_over=dict(probe_deep_begin=8))
+    assert hb.hermes_last_score_path(ls.h) == hb.HERMES_SCORE_TCGEN05
+    ls.close()
