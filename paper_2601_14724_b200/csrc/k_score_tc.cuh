@@ -595,7 +595,7 @@ struct TcState {
   std::string trace_path;
   void (*k_score)(CUtensorMap, CUtensorMap, TcArgs) = nullptr;
   unsigned seg_total = 0;       // running target of the pass-1 progress counters (wraps; compared wrap-safe)
-  int var1 = 0, var2 = 0;   // experiment switches (HERMES_TC_VAR1 / HERMES_TC_VAR2)
+  int var1 = 0;             // diagnostics: HERMES_TC_VAR1 = 1 interleaved exp loop, 3 = + 1/8 of the exp2 on the FMA pipe
 };
 
 // 2D bf16 tensor map over [rows][cols] (cols contiguous), 64 x 64 boxes, 128-byte swizzle, zero OOB fill.
@@ -631,7 +631,6 @@ inline bool tc_init(hermes_t* h) {
     if (cudaMalloc(&st->trace, 2 * kTcTraceStride * 8) != cudaSuccess) st->trace = nullptr;
   }
   if (const char* e = getenv("HERMES_TC_VAR1")) st->var1 = atoi(e);
-  if (const char* e = getenv("HERMES_TC_VAR2")) st->var2 = atoi(e);
   const Geom& g = h->geom;
   if (!tc_make_map(st, &st->tmap_k, g.kc, uint64_t(g.row_elems), uint64_t(g.B) * g.L * 2 * g.cap)) {
     h->err = "cuTensorMapEncodeTiled(K cache) failed"; delete st; return false;
