@@ -702,15 +702,16 @@ inline int tc_score(hermes_t* h, const void* q_probe, int Tn, int P, float scale
   a.q_half_bytes = (a.RS + 63) / 64 * 8192;
   a.n_kst = std::min(kTcKStagesMax, (kTcSmemMax - tc_smem_bytes(a.q_half_bytes, 0)) / kTcKStage);
   const int smem = tc_smem_bytes(a.q_half_bytes, a.n_kst);
-  st->seg_total += unsigned(a.spg) * kTcEpiWarps;
+  // pass 2 waits until the group's counter reaches this value; committed only once the launch has succeeded
   a.seg_cnt = reinterpret_cast<unsigned*>(h->ws + h->lay.seg_cnt);
-  a.seg_target = st->seg_total;
+  a.seg_target = st->seg_total + unsigned(a.spg) * kTcEpiWarps;
   {
     TcProf p(h, HERMES_K_SCORE_STATS, s);
     a.trace = st->trace;
     if (st->trace) cudaMemsetAsync(st->trace, 0, 2 * kTcTraceStride * 8, s);
     const cudaError_t e = launch_pdl(st->k_score, dim3(n_cta), dim3(kTcThreads), size_t(smem), s, tmap_q, st->tmap_k, a);
     if (e != cudaSuccess) { h->err = std::string("tcgen05 scoring launch: ") + cudaGetErrorString(e); return HERMES_ECUDA; }
+    st->seg_total = a.seg_target;
   }
   return HERMES_OK;
 }
