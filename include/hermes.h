@@ -88,6 +88,10 @@ typedef struct {
                                    token of the evicted ones (Alg. 1) in slot budget-1 at
                                    position pos_offset+budget-1; last_kept[budget-1] = -1 marks it.  Needs
                                    HERMES_ROPE_1D and HERMES_REINDEX_EAGER                              */
+  int32_t defer_v;              /* 1 (default): on the tcgen05 path an eviction compacts K at once but leaves the
+                                   kept V rows to be moved by the NEXT update's scoring kernel (V is not read by
+                                   scoring, so the copy hides behind it); hermes_get_cache() and updates that do
+                                   not score on tcgen05 first run the pending move on their own.  0: never defer */
   int32_t score_path;           /* HERMES_SCORE_*: AUTO picks tcgen05 when the contraction is dense */
   int32_t device;               /* CUDA device ordinal                                         */
 } hermes_config;
@@ -138,7 +142,8 @@ int hermes_append_chunk_host(hermes_t *h, const void *K_new_host, const void *V_
                              const void *Q_probe_host, int32_t n_new, int32_t n_probe,
                              int32_t pos_start, int32_t *kept_out_host, void *cuda_stream);
 
-/* Fills *out for (stream, layer).  No synchronisation.                                               */
+/* Fills *out for (stream, layer).  No synchronisation; if a V compaction is pending (defer_v) it is enqueued
+ * on the stream of the last append first.                                                              */
 int hermes_get_cache(hermes_t *h, int32_t stream, int32_t layer, hermes_cache_view *out);
 
 /* Host-tracked token count per layer (same for every stream and layer).                              */

@@ -37,7 +37,7 @@ class HermesConfig(C.Structure):
                 ("rope_theta", C.c_float), ("mrope_section", C.c_int32 * 3),
                 ("mrope_compact_axes", C.c_int32), ("mrope_grid_h", C.c_int32),
                 ("mrope_grid_w", C.c_int32), ("pos_offset", C.c_int32), ("reindex_mode", C.c_int32),
-                ("max_position", C.c_int32), ("probe_deep_begin", C.c_int32), ("summary_token", C.c_int32), ("score_path", C.c_int32),
+                ("max_position", C.c_int32), ("probe_deep_begin", C.c_int32), ("summary_token", C.c_int32), ("defer_v", C.c_int32), ("score_path", C.c_int32),
                 ("device", C.c_int32)]
 
 

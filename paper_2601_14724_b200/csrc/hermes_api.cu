@@ -14,6 +14,11 @@ using namespace hk;
 
 static thread_local std::string g_create_error;
 
+namespace {
+template <typename T> struct TypeTag { using type = T; };
+void flush_v(hermes_t* h, cudaStream_t s);   // runs a deferred V compaction on its own
+}  // namespace
+
 static int fail(hermes_t* h, int code, const char* fmt, ...) {
   char buf[512];
   va_list ap;
@@ -45,6 +50,7 @@ extern "C" void hermes_default_config(hermes_config* c) {
   c->max_probe_tokens = 64;
   c->score_path = HERMES_SCORE_AUTO;
   c->reindex_mode = HERMES_REINDEX_EAGER;
+  c->defer_v = 1;
 }
 
 extern "C" size_t hermes_workspace_bytes(const hermes_config* c) {
@@ -214,6 +220,11 @@ extern "C" int hermes_get_cache(hermes_t* h, int32_t stream, int32_t layer, herm
   if (stream < 0 || stream >= h->cfg.n_streams || layer < 0 || layer >= h->cfg.n_layers)
     return fail(h, HERMES_EINVAL, "stream %d / layer %d out of range", stream, layer);
   const Geom& g = h->geom;
+  if (h->v_pending) {                       // make V whole before handing out pointers (stream of the last append)
+    flush_v(h, static_cast<cudaStream_t>(h->last_stream));
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(h, HERMES_ECUDA, "V compaction: %s", cudaGetErrorString(e));
+  }
   const size_t bl = size_t(stream) * g.L + layer, slab = bl * 2 + h->cur;
   out->k = static_cast<char*>(g.kc) + slab * g.cap * h->lay.row_bytes;
   out->v = static_cast<char*>(g.vc) + slab * g.cap * h->lay.row_bytes;
@@ -255,6 +266,43 @@ void launch_simt(hermes_t* h, const void* q, int Tn, int P, float scale_log2, cu
   else if (g.d == 64) run(std::integral_constant<int, 64>{});
   else run(std::integral_constant<int, 128>{});
 }
+// k_gather for buffer `buf` -> buf ^ 1 in the given mode (kGatherKV / kGatherK / kGatherV).
+void launch_gather(hermes_t* h, int mode, int buf, cudaStream_t s) {
+  const hermes_config& c = h->cfg;
+  const Geom& g = h->geom;
+  const int BL = g.B * g.L;
+  const int V = c.dtype == HERMES_BF16 ? 8 : 4;
+  const int upr = g.Hkv * (g.d / 2 / V);
+  const int total = g.budget * upr;
+  // 4 resident blocks per SM; 8 whole waves over all slabs measured best (118 -> 114 us at configs[1]; a
+  // partial extra wave, as the old rounding produced, cost 5 us): short blocks even out the per-SM HBM rates
+  const int want = std::max(1, (h->n_sm * 4 * 8) / BL);
+  const int gx = std::max(1, std::min(want, (total + kGatherThreads - 1) / kGatherThreads));
+  const dim3 grid(gx, BL), block(kGatherThreads);
+  auto go = [&](auto tag, auto nax, auto md) {
+    using T = typename decltype(tag)::type;
+    launch_pdl(k_gather<T, decltype(nax)::value, decltype(md)::value>, grid, block, 0, s, g, buf);
+  };
+  auto by_mode = [&](auto tag, auto nax) {
+    if (mode == kGatherKV) go(tag, nax, std::integral_constant<int, kGatherKV>{});
+    else if (mode == kGatherK) go(tag, nax, std::integral_constant<int, kGatherK>{});
+    else go(tag, nax, std::integral_constant<int, kGatherV>{});
+  };
+  auto by_axes = [&](auto tag) {
+    if (g.n_axes == 1) by_mode(tag, std::integral_constant<int, 1>{});
+    else by_mode(tag, std::integral_constant<int, 3>{});
+  };
+  if (c.dtype == HERMES_BF16) by_axes(TypeTag<__nv_bfloat16>{});
+  else by_axes(TypeTag<float>{});
+}
+
+// Runs a deferred V compaction on its own (no scoring kernel to carry it).
+void flush_v(hermes_t* h, cudaStream_t s) {
+  if (!h->v_pending) return;
+  launch_gather(h, kGatherV, h->v_src_buf, s);
+  ++h->last_launches;
+  h->v_pending = false;
+}
 }  // namespace
 
 extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V_new, const void* Q_probe,
@@ -295,6 +343,10 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
   for (bool& r : h->timer.ran) r = false;
   const int row_vecs = int(h->lay.row_bytes / 16);
   const int BL = g.B * g.L;
+  const bool use_tc = evict && g.L > g.n_shallow && h->tc_ok && c.score_path != HERMES_SCORE_SIMT &&
+                      (c.score_path == HERMES_SCORE_TCGEN05 || tc_profitable(h, Tn, n_probe));
+  h->last_stream = cuda_stream;
+  if (!use_tc) flush_v(h, s);               // no scoring kernel to carry a pending V compaction
   {
     Prof p(h, HERMES_K_APPEND, s);
     const size_t n_vec = size_t(n_new) * row_vecs;
@@ -306,10 +358,9 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
     const float scale = c.softmax_scale > 0.f ? c.softmax_scale : float(1.0 / std::sqrt(double(c.head_dim)));
     const float scale_log2 = scale * kLog2e;
     if (g.L > g.n_shallow) {
-      const bool use_tc = h->tc_ok && c.score_path != HERMES_SCORE_SIMT &&
-                          (c.score_path == HERMES_SCORE_TCGEN05 || tc_profitable(h, Tn, n_probe));
       if (use_tc) {
-        if (int rc = tc_score(h, Q_probe, Tn, n_probe, scale_log2, s)) return rc;
+        if (int rc = tc_score(h, Q_probe, Tn, n_probe, scale_log2, s, h->v_pending)) return rc;
+        h->v_pending = false;
         h->last_score_path = HERMES_SCORE_TCGEN05;
       } else {
         if (c.dtype == HERMES_BF16) launch_simt<__nv_bfloat16>(h, Q_probe, Tn, n_probe, scale_log2, s);
@@ -336,21 +387,10 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
     }
     {
       Prof p(h, HERMES_K_GATHER, s);
-      const int V = c.dtype == HERMES_BF16 ? 8 : 4;
-      const int upr = g.Hkv * (g.d / 2 / V);
-      const int total = g.budget * upr;
-      // 4 resident blocks per SM; 8 whole waves over all slabs measured best (118 -> 114 us at configs[1]; a
-      // partial extra wave, as the old rounding produced, cost 5 us): short blocks even out the per-SM HBM rates
-      const int want = std::max(1, (h->n_sm * 4 * 8) / BL);
-      const int gx = std::max(1, std::min(want, (total + kGatherThreads - 1) / kGatherThreads));
-      const dim3 grid(gx, BL);
-      if (c.dtype == HERMES_BF16) {
-        if (g.n_axes == 1) launch_pdl(k_gather<__nv_bfloat16, 1>, grid, dim3(kGatherThreads), 0, s, g, h->cur);
-        else launch_pdl(k_gather<__nv_bfloat16, 3>, grid, dim3(kGatherThreads), 0, s, g, h->cur);
-      } else {
-        if (g.n_axes == 1) launch_pdl(k_gather<float, 1>, grid, dim3(kGatherThreads), 0, s, g, h->cur);
-        else launch_pdl(k_gather<float, 3>, grid, dim3(kGatherThreads), 0, s, g, h->cur);
-      }
+      // on the tcgen05 path V stays behind: the next update's scoring kernel compacts it (tc_v_mover), or a flush
+      const bool defer_v = use_tc && c.defer_v != 0;
+      launch_gather(h, defer_v ? kGatherK : kGatherKV, h->cur, s);
+      if (defer_v) { h->v_pending = true; h->v_src_buf = h->cur; }
     }
   }
   cudaError_t e = cudaGetLastError();

@@ -59,6 +59,7 @@ inline const char* validate(const hermes_config& c) {
   if (c.pos_offset < 0) return "pos_offset must be >= 0";
   if (c.reindex_mode != HERMES_REINDEX_EAGER && c.reindex_mode != HERMES_REINDEX_LAZY) return "bad reindex_mode";
   if (c.probe_deep_begin < 0 || c.probe_deep_begin >= c.max_probe_tokens) return "probe_deep_begin must lie in [0, max_probe_tokens)";
+  if (c.defer_v != 0 && c.defer_v != 1) return "defer_v must be 0 or 1";
   if (c.summary_token != 0 && c.summary_token != 1) return "summary_token must be 0 or 1";
   if (c.summary_token && (c.rope_mode != HERMES_ROPE_1D || c.reindex_mode != HERMES_REINDEX_EAGER || c.budget < 2))
     return "summary tokens need 1D RoPE, eager re-indexing and budget >= 2";
@@ -158,6 +159,11 @@ struct hermes {
   int last_launches = 0;
   int n_sm = 148;
   int n_vh = 0;             // column-sum slots written by the last scoring pass
+  // deferred V compaction: after an eviction on the tcgen05 path k_gather moves only K; the kept V rows still sit
+  // in buffer v_src_buf and are moved into the current buffer by the NEXT update's scoring kernel (or by a flush)
+  bool v_pending = false;
+  int v_src_buf = 0;
+  void* last_stream = nullptr;
   bool profiling = false;
   bool tc_ok = false;       // tcgen05 scoring path usable for this config + device
   hk::KernelTimer timer;

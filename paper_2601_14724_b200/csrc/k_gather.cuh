@@ -73,7 +73,11 @@ __device__ __forceinline__ void rotate_unit(const Geom& g, const int (&dl)[NAX],
 }
 
 // grid = (blocks per slab, B*L); each thread walks units idx, idx + stride, ... of its (stream, layer).
-template <typename T, int NAX>
+// kMode: kGatherKV moves K and V; kGatherK only K (V's compaction is deferred into the next update's scoring
+// kernel, see tc_v_mover in k_score_tc.cuh); kGatherV only V (flush of a deferred compaction).
+constexpr int kGatherKV = 0, kGatherK = 1, kGatherV = 2;
+
+template <typename T, int NAX, int kMode>
 __global__ void __launch_bounds__(kGatherThreads, 4)
 k_gather(Geom g, int cur) {
   pdl_wait();
@@ -92,44 +96,65 @@ k_gather(Geom g, int cur) {
   const int32_t* kept = g.kept + size_t(bl) * g.budget;
   const int32_t* delta = g.delta + size_t(bl) * g.n_axes * g.budget;   // written by k_select
 
+  // units per trip: 1 everywhere.  (K-only mode with 2-4 units per trip, or with 5-6 blocks per SM, measured slower:
+  // 81-99 us against 72 us -- register spills at 64 registers, fewer resident blocks above that.)
+  constexpr int UPT = 1;
   const int stride = gridDim.x * kGatherThreads;
-  int idx = blockIdx.x * kGatherThreads + threadIdx.x;
-  if (idx >= total) return;
-  int s = idx / upr;
-  int src = __ldcg(kept + s);
-  int dl[NAX];
+  int idx[UPT], s[UPT], src[UPT], dl[UPT][NAX];
 #pragma unroll
-  for (int a = 0; a < NAX; ++a) dl[a] = __ldcg(delta + a * g.budget + s);
+  for (int p = 0; p < UPT; ++p) {
+    idx[p] = blockIdx.x * kGatherThreads + threadIdx.x + p * stride;
+    s[p] = min(idx[p], total - 1) / upr;
+    src[p] = __ldcg(kept + s[p]);
+#pragma unroll
+    for (int a = 0; a < NAX; ++a) dl[p][a] = __ldcg(delta + a * g.budget + s[p]);
+  }
+  if (idx[0] >= total) return;
 
 #pragma unroll 1
   while (true) {
-    const int u = idx - s * upr;
-    const int e = (u / uph) * g.d + (u % uph) * V;
-    const size_t so = size_t(max(src, 0)) * g.row_elems + e;   // src < 0: the summary-token slot, written by k_summary
-    uint4 klo = ldg_stream(ks + so), khi = ldg_stream(ks + so + half);
-    const uint4 vlo = ldg_stream(vs + so), vhi = ldg_stream(vs + so + half);
-    // prefetch the next step's row index and deltas
-    const int idx_n = idx + stride;
-    const bool more = idx_n < total;
-    const int s_n = more ? idx_n / upr : s;
-    const int src_n = __ldcg(kept + s_n);
-    int dl_n[NAX];
+    uint4 klo[UPT], khi[UPT], vlo[UPT], vhi[UPT];
+    int e[UPT], j0[UPT];
 #pragma unroll
-    for (int a = 0; a < NAX; ++a) dl_n[a] = __ldcg(delta + a * g.budget + s_n);
-
-    bool any = false;
-#pragma unroll
-    for (int a = 0; a < NAX; ++a) any |= dl[a] != 0;
-    if (any) rotate_unit<T, NAX>(g, dl, (u % uph) * V, klo, khi);
-    const size_t dof = size_t(s) * g.row_elems + e;
-    if (src >= 0) {
-      stg_stream(kd + dof, klo); stg_stream(kd + dof + half, khi);
-      stg_stream(vd + dof, vlo); stg_stream(vd + dof + half, vhi);
+    for (int p = 0; p < UPT; ++p) {
+      const int u = min(idx[p], total - 1) - s[p] * upr;
+      e[p] = (u / uph) * g.d + (u % uph) * V;
+      j0[p] = (u % uph) * V;
+      const size_t so = size_t(max(src[p], 0)) * g.row_elems + e[p];   // src < 0: the summary-token slot, written by k_summary
+      klo[p] = khi[p] = vlo[p] = vhi[p] = make_uint4(0, 0, 0, 0);
+      if (kMode != kGatherV) { klo[p] = ldg_stream(ks + so); khi[p] = ldg_stream(ks + so + half); }
+      if (kMode != kGatherK) { vlo[p] = ldg_stream(vs + so); vhi[p] = ldg_stream(vs + so + half); }
     }
-    if (!more) break;
-    idx = idx_n; s = s_n; src = src_n;
+    // prefetch the next trip's row indices and deltas
+    int idx_n[UPT], s_n[UPT], src_n[UPT], dl_n[UPT][NAX];
 #pragma unroll
-    for (int a = 0; a < NAX; ++a) dl[a] = dl_n[a];
+    for (int p = 0; p < UPT; ++p) {
+      idx_n[p] = idx[p] + UPT * stride;
+      s_n[p] = min(idx_n[p], total - 1) / upr;
+      src_n[p] = __ldcg(kept + s_n[p]);
+#pragma unroll
+      for (int a = 0; a < NAX; ++a) dl_n[p][a] = __ldcg(delta + a * g.budget + s_n[p]);
+    }
+#pragma unroll
+    for (int p = 0; p < UPT; ++p) {
+      if (idx[p] >= total) continue;
+      bool any = false;
+#pragma unroll
+      for (int a = 0; a < NAX; ++a) any |= dl[p][a] != 0;
+      if (kMode != kGatherV && any) rotate_unit<T, NAX>(g, dl[p], j0[p], klo[p], khi[p]);
+      const size_t dof = size_t(s[p]) * g.row_elems + e[p];
+      if (src[p] >= 0) {
+        if (kMode != kGatherV) { stg_stream(kd + dof, klo[p]); stg_stream(kd + dof + half, khi[p]); }
+        if (kMode != kGatherK) { stg_stream(vd + dof, vlo[p]); stg_stream(vd + dof + half, vhi[p]); }
+      }
+    }
+    if (idx_n[0] >= total) break;
+#pragma unroll
+    for (int p = 0; p < UPT; ++p) {
+      idx[p] = idx_n[p]; s[p] = s_n[p]; src[p] = src_n[p];
+#pragma unroll
+      for (int a = 0; a < NAX; ++a) dl[p][a] = dl_n[p][a];
+    }
   }
 }
 

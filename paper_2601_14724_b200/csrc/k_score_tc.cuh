@@ -27,7 +27,8 @@ constexpr int kTcKStage = kTcTile * 256;        // bytes per K tile: 128 tokens 
 constexpr int kTcKStagesMax = 4;                // K ring depth: as many 32 KB stages as fit beside the Q rows
 constexpr int kTcSmemMax = 232448;              // 227 KB dynamic shared memory per CTA
 constexpr int kTcEpiWarps = 16;                 // epilogue warps: 4 per SM sub-partition / TMEM lane quarter
-constexpr int kTcThreads = 64 + kTcEpiWarps * 32;   // producer, MMA, epilogue
+constexpr int kTcThreads = 64 + kTcEpiWarps * 32 + 32;   // producer, MMA, epilogue, V mover
+constexpr int kTcMoverRing = 32768;             // shared-memory staging of the V mover
 constexpr int kTcSegTiles = 4;                  // pass 1: 128-token tiles per segment (one partial pair per
                                                 // segment, so the merge order never depends on the CTA schedule)
 
@@ -41,6 +42,10 @@ struct TcArgs {
   int spg;                  // pass 1: 512-token segments per group = partial (m, z) slots per probe row
   int q_half_bytes;         // shared-memory bytes of one 64-column half of the group's Q rows (64-row boxes)
   int n_kst;                // K ring stages
+  // deferred V compaction of the PREVIOUS update, moved by one warp per CTA while this update is scored
+  const char* v_base;       // V cache base, or NULL: nothing pending
+  const int32_t* v_kept;    // [B*L][budget] kept lists of the previous update
+  int v_src_buf, v_row_bytes;
   unsigned* seg_cnt;        // [n_groups] pass-1 progress: += 16 (epilogue warps) per finished segment, never reset
   unsigned seg_target;      // value of seg_cnt[g] once all pass-1 segments of THIS update are done
   long long* trace;         // optional event trace of CTA 0 (HERMES_TC_TRACE; NULL in production)
@@ -81,18 +86,20 @@ struct TcSmem {
   uint8_t* k;        // K ring: [stage][2 halves][128 tokens][128 B]
   float* c;          // [512] per-row c_r (pass 2)
   float4* xch;       // [2][8][32] pass-1 exchange between the two token-half warps of a row block quarter
+  uint8_t* ring;     // V mover staging (kTcMoverRing bytes; only when a compaction is pending)
   float2* xch2;      // [2][2][32] pass-1 exchange between the even- / odd-tile lane quarters of a half-full row block
   uint64_t* bars;    // mbarriers
   uint32_t* tmem;    // TMEM base address written by tcgen05.alloc
 };
-__host__ __device__ inline int tc_smem_bytes(int q_half_bytes, int n_kst) {
-  return 1024 + 2 * q_half_bytes + n_kst * kTcKStage + kTcRowsMax * 4 + 8192 + 1024 + 256 + 16;
+__host__ __device__ inline int tc_smem_bytes(int q_half_bytes, int n_kst, bool mover) {
+  return (mover ? kTcMoverRing : 0) + 1024 + 2 * q_half_bytes + n_kst * kTcKStage + kTcRowsMax * 4 + 8192 + 1024 + 256 + 16;
 }
 __device__ inline TcSmem tc_carve(uint8_t* raw, const TcArgs& a) {
   uint8_t* p = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(raw) + 1023) & ~uintptr_t(1023));
   TcSmem s;
   s.q = p; p += 2 * a.q_half_bytes;
   s.k = p; p += a.n_kst * kTcKStage;
+  s.ring = p; p += a.v_base ? kTcMoverRing : 0;
   s.c = reinterpret_cast<float*>(p); p += kTcRowsMax * 4;
   s.xch = reinterpret_cast<float4*>(p); p += 8192;
   s.xch2 = reinterpret_cast<float2*>(p); p += 1024;
@@ -102,13 +109,13 @@ __device__ inline TcSmem tc_carve(uint8_t* raw, const TcArgs& a) {
 }
 
 struct TcBars {
-  uint64_t *k_full, *k_empty, *t_full, *t_empty, *q_full, *q_empty;
+  uint64_t *k_full, *k_empty, *t_full, *t_empty, *q_full, *q_empty, *v_full;
 };
 __device__ inline TcBars tc_bars(const TcSmem& s) {
   TcBars b;
   b.k_full = s.bars; b.k_empty = s.bars + kTcKStagesMax;
   b.t_full = s.bars + 2 * kTcKStagesMax; b.t_empty = b.t_full + 2;
-  b.q_full = b.t_empty + 2; b.q_empty = b.q_full + 1;
+  b.q_full = b.t_empty + 2; b.q_empty = b.q_full + 1; b.v_full = b.q_empty + 1;
   return b;
 }
 __device__ inline uint32_t tc_prologue(const TcSmem& s, const TcBars& b, const TcArgs& a, const CUtensorMap* tq, const CUtensorMap* tk) {
@@ -117,7 +124,7 @@ __device__ inline uint32_t tc_prologue(const TcSmem& s, const TcBars& b, const T
     ptx::prefetch_tmap(tq); ptx::prefetch_tmap(tk);
     for (int i = 0; i < a.n_kst; ++i) { ptx::mbar_init(&b.k_full[i], 1); ptx::mbar_init(&b.k_empty[i], 1); }
     for (int i = 0; i < 2; ++i) { ptx::mbar_init(&b.t_full[i], 1); ptx::mbar_init(&b.t_empty[i], kTcEpiWarps); }
-    ptx::mbar_init(b.q_full, 1); ptx::mbar_init(b.q_empty, 1);
+    ptx::mbar_init(b.q_full, 1); ptx::mbar_init(b.q_empty, 1); ptx::mbar_init(b.v_full, 1);
     ptx::fence_barrier_init();
   }
   if (warp == 1) ptx::tmem_alloc(s.tmem, 512);
@@ -244,7 +251,7 @@ __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const
       if (++x == a.spg) { x = 0; g.next(a); new_group = true; }
     }
     st.ks = ks; st.kph = kph; st.as = as; st.aph = aph; st.n_q = n_q;
-  } else {
+  } else if (warp < 2 + kTcEpiWarps) {
     // ---------------- epilogue: one probe row x 64 tokens per thread per stage ----------------
     const int e = warp - 2, rbl = e >> 3, th = (e >> 2) & 1, lg = warp & 3;
     const uint32_t t_addr = tmem_base + (uint32_t(lg * 32) << 16) + rbl * kTcTile + th * 64;
@@ -453,7 +460,7 @@ __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const
       if (++ks == a.n_kst) { ks = 0; kph ^= 1; }
       if (++t == a.tpg) { t = 0; g.next(a); new_group = true; }
     }
-  } else {
+  } else if (warp < 2 + kTcEpiWarps) {
     // ---------------- epilogue: one token per thread; warp (lane quarter lg, column quarter cq) ----------------
     const int e = warp - 2, cq = e >> 2, lg = warp & 3;
     const int tok_in_tile = lg * 32 + lane;
@@ -549,6 +556,43 @@ __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const
   }
 }
 
+// V mover (warp 2 + kTcEpiWarps): compaction of V needs no arithmetic and nothing in the scoring of the NEXT update
+// reads V, so k_gather leaves V behind and this warp moves the kept rows V[kept[s]] -> V'[s] of the previous update
+// with 1D bulk copies (global -> shared -> global) while the tensor / XU pipes score: one row per lane, one
+// mbarrier wait per batch.  The CTA's share is ~1200 rows of 1 KB over ~200 us: a few GB/s per SM.
+__device__ inline void tc_v_mover(const TcSmem& s, const TcBars& b, const TcArgs& a) {
+  const int lane = threadIdx.x & 31;
+  const int budget = a.g.budget, rb = a.v_row_bytes;
+  const int per = min(32, kTcMoverRing / rb);                             // rows per batch
+  const long long n_rows = (long long)a.g.B * a.g.L * budget;
+  const long long r0 = n_rows * blockIdx.x / gridDim.x, r1 = n_rows * (blockIdx.x + 1) / gridDim.x;
+  int bl = int(r0 / budget), sl = int(r0 - (long long)bl * budget) + lane;   // this lane's (slab, slot); no division below
+  int ph = 0;
+  for (long long i0 = r0; i0 < r1; i0 += per) {
+    while (sl >= budget) { sl -= budget; ++bl; }
+    const bool on = lane < per && i0 + lane < r1;
+    int src = -1;
+    if (on) src = __ldcg(a.v_kept + size_t(bl) * budget + sl);            // < 0: summary-token slot, not a copy
+    const unsigned m = __ballot_sync(0xffffffffu, on && src >= 0);
+    if (m != 0) {
+      if (lane == 0) ptx::mbar_expect_tx(b.v_full, uint32_t(__popc(m)) * rb);
+      __syncwarp();
+      uint8_t* slot = s.ring + lane * rb;
+      if (on && src >= 0)
+        ptx::bulk_load(slot, a.v_base + ((size_t(bl) * 2 + a.v_src_buf) * a.g.cap + src) * rb, rb, b.v_full);
+      ptx::mbar_wait(b.v_full, ph); ph ^= 1;
+      if (on && src >= 0) {
+        ptx::bulk_store(const_cast<char*>(a.v_base) + ((size_t(bl) * 2 + (a.v_src_buf ^ 1)) * a.g.cap + sl) * rb, slot, rb);
+        ptx::bulk_commit();
+      }
+      ptx::bulk_wait_read0();                                             // staging slots may be overwritten
+      __syncwarp();
+    }
+    sl += per;
+  }
+  ptx::bulk_wait0();                                                      // every row is in global memory
+}
+
 // =====================================================================================================
 // One persistent kernel runs both passes: every CTA works through its pass-1 range, then its pass-2
 // range of the same flattened (group, token) space, keeping TMEM, barriers and the K ring alive.  Pass 2
@@ -565,6 +609,7 @@ k_tc_score(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ C
   const uint32_t tmem_base = tc_prologue(s, b, a, &tmap_q, &tmap_k);
   pdl_wait();                       // the chunk's K rows come from k_append
   if (threadIdx.x == 0) pdl_launch_dependents();
+  if ((threadIdx.x >> 5) == 2 + kTcEpiWarps && a.v_base != nullptr) tc_v_mover(s, b, a);
   TcRole st;
   tc_pass1<kVar, kTrace>(s, b, &tmap_q, &tmap_k, a, tmem_base, st);
   if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.trace[4 * kTcTraceN + 2 * blockIdx.x + 1] = t; }
@@ -676,7 +721,7 @@ struct TcProf {   // same event bracketing as hermes_api.cu's Prof, local to thi
   ~TcProf() { if (h->profiling) cudaEventRecord(h->timer.end[id], s); }
 };
 
-inline int tc_score(hermes_t* h, const void* q_probe, int Tn, int P, float scale_log2, cudaStream_t s) {
+inline int tc_score(hermes_t* h, const void* q_probe, int Tn, int P, float scale_log2, cudaStream_t s, bool move_v) {
   TcState* st = static_cast<TcState*>(h->tc_state);
   const Geom& g = h->geom;
   CUtensorMap tmap_q;
@@ -700,8 +745,12 @@ inline int tc_score(hermes_t* h, const void* q_probe, int Tn, int P, float scale
   if (a.spg > h->lay.n_part_max || g.Hkv * a.n_sc * 4 > g.n_vh_max) { h->err = "internal: tc scratch too small"; return HERMES_ESTATE; }
   h->n_vh = g.Hkv * a.n_sc * 4;
   a.q_half_bytes = (a.RS + 63) / 64 * 8192;
-  a.n_kst = std::min(kTcKStagesMax, (kTcSmemMax - tc_smem_bytes(a.q_half_bytes, 0)) / kTcKStage);
-  const int smem = tc_smem_bytes(a.q_half_bytes, a.n_kst);
+  // a pending V compaction of the previous update rides in this launch (tc_v_mover)
+  a.v_base = move_v ? static_cast<const char*>(g.vc) : nullptr;
+  a.v_kept = g.kept; a.v_src_buf = h->v_src_buf; a.v_row_bytes = int(h->lay.row_bytes);
+  a.n_kst = std::min(kTcKStagesMax, (kTcSmemMax - tc_smem_bytes(a.q_half_bytes, 0, move_v)) / kTcKStage);
+  if (a.n_kst < 2) { h->err = "tcgen05 scoring: shared memory too small for the K ring"; return HERMES_ESTATE; }
+  const int smem = tc_smem_bytes(a.q_half_bytes, a.n_kst, move_v);
   // pass 2 waits until the group's counter reaches this value; committed only once the launch has succeeded
   a.seg_cnt = reinterpret_cast<unsigned*>(h->ws + h->lay.seg_cnt);
   a.seg_target = st->seg_total + unsigned(a.spg) * kTcEpiWarps;

@@ -225,3 +225,32 @@ def test_probe_row_ranges_simt_and_tcgen05():
     ls, _ = _run(wl, 2, n_warm=1, cfg_over=dict(probe_deep_begin=8), oracle_over=dict(probe_deep_begin=8))
     assert hb.hermes_last_score_path(ls.h) == hb.HERMES_SCORE_TCGEN05
     ls.close()
+
+
+def test_deferred_v_compaction_equals_immediate():
+    """defer_v: V rows moved by the next update's scoring kernel (tc_v_mover) or by a flush must give the same cache,
+    bit for bit, as compacting V at once; the summary-token slot and a SIMT-path update in between are covered."""
+    wl = CONFIGS["llava_ov_7b"].scaled(n_layers=7, budget=784, probe_tokens=16)
+
+    def run(defer, summary):
+        ls = LockStep(wl, cfg_over=dict(defer_v=defer, summary_token=summary), oracle_over=dict(summary_token=bool(summary)))
+        ls.fill()
+        for i in range(5):
+            ls.step(check=False)                                 # deferred moves ride in the next scoring kernel
+        ls.step(check=False, n_probe=2)                          # G*P = 14 < 32: CUDA-core path -> flush before append
+        ls.step(check=False)
+        torch.cuda.synchronize()
+        out = [{k: t.clone() for k, t in hb.hermes_get_cache(ls.h, 0, l).items() if torch.is_tensor(t)}
+               for l in range(wl.n_layers)]                      # get_cache flushes the last pending move
+        assert hb.hermes_device_status(ls.h) == 0
+        ls.close()
+        return out
+
+    for summary in (0, 1):
+        a, b = run(1, summary), run(0, summary)
+        for l in range(wl.n_layers):
+            for key in ("k", "v", "pos", "last_kept", "last_scores"):
+                assert torch.equal(a[l][key], b[l][key]), (summary, l, key)
+    # and the lock-step oracle comparison still holds when every checked update starts from a flushed cache
+    ls, reps = _run(wl, 3, n_warm=2, cfg_over=dict(defer_v=1))
+    ls.close()
