@@ -27,8 +27,9 @@ from workloads import CONFIGS, chunk_kv, probe_q, sweep_point  # noqa: E402
 METRIC, UNIT = "kv_tokens_managed_per_s", "tokens/s"
 POOL = 16          # distinct pre-generated chunk/probe sets cycled through the timed region
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at configs[1], transcribed from the one
-# `ncu --set full` capture summarised in profiles/r1c_ncu_full_summary.txt (command in profiles/r1c_README.md)
-NCU_TRAFFIC_BYTES = {"gather": 361.18e6 + 309.93e6, "score": 367.49e6 + 15.54e6,
+# `ncu --set full` capture summarised in profiles/r1d_ncu_full_summary.txt (command in profiles/r1d_README.md);
+# the scoring kernel's figure includes the previous update's V compaction (360 MB) that rides in it
+NCU_TRAFFIC_BYTES = {"gather": 181.35e6 + 131.55e6, "score": 563.21e6 + 192.38e6,
                      "select": 1.44e6, "append": 11.25e6}
 
 
@@ -65,7 +66,7 @@ class ClockSampler:
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                       "--format=csv,noheader,nounits", "-lms", "20"],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
@@ -236,7 +237,7 @@ def run_ours(args):
     t_dom = kern[dom] * 1e-3
     traffic = NCU_TRAFFIC_BYTES.get(dom) if args.workload == "llava_ov_7b" else None
     if dom == "gather" or dom == "append":
-        ach = work["gather_bytes"] / t_dom / 1e9
+        ach = work["gather_bytes"] / 2 / t_dom / 1e9          # K-only launch (V is moved inside the scoring kernel)
         roof = dict(kernel=dom, bound="hbm", achieved=ach, peak=pk["hbm"], unit="GB/s", frac=ach / pk["hbm"], traffic=traffic)
     elif dom == "score":
         # exp2-bound: both passes evaluate one exp2 per (probe row, token) on the XU pipe,
@@ -335,7 +336,7 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=1024)
+    ap.add_argument("--steps", type=int, default=256)   # BASELINE.json configs[1]: 256 timed chunk arrivals
     ap.add_argument("--warmup", type=int, default=8)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="llava_ov_7b", help="one of %s, or sweep:<budget>:<probe>" % sorted(CONFIGS))
