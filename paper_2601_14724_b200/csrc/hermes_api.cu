@@ -274,9 +274,10 @@ void launch_gather(hermes_t* h, int mode, int buf, cudaStream_t s) {
   const int V = c.dtype == HERMES_BF16 ? 8 : 4;
   const int upr = g.Hkv * (g.d / 2 / V);
   const int total = g.budget * upr;
-  // 4 resident blocks per SM; 8 whole waves over all slabs measured best (118 -> 114 us at configs[1]; a
-  // partial extra wave, as the old rounding produced, cost 5 us): short blocks even out the per-SM HBM rates
-  const int want = std::max(1, (h->n_sm * 4 * 8) / BL);
+  // 4 resident blocks per SM, whole waves only (a partial extra wave, as the old rounding produced, cost 5 us);
+  // K + V launches: 8 waves measured best (118 -> 114 us at configs[1]: short blocks even out the per-SM HBM rates)
+  const int waves = mode == kGatherK ? 2 : 8;     // the K-only launch prefers long blocks: 69.6 us at 2 waves, 72.2 at 8, 81 at 24
+  const int want = std::max(1, (h->n_sm * 4 * waves) / BL);
   const int gx = std::max(1, std::min(want, (total + kGatherThreads - 1) / kGatherThreads));
   const dim3 grid(gx, BL), block(kGatherThreads);
   auto go = [&](auto tag, auto nax, auto md) {
