@@ -164,6 +164,9 @@ int hermes_get_profile(hermes_t *h, float *ms_out, int32_t n);
 /* Which scoring path the last eviction used: HERMES_SCORE_SIMT or HERMES_SCORE_TCGEN05 (0 if none).  */
 int32_t hermes_last_score_path(const hermes_t *h);
 
+/* 1 if a V compaction is pending (defer_v): the kept V rows of the last eviction have not been moved yet.        */
+int32_t hermes_v_pending(const hermes_t *h);
+
 /* Number of kernels launched by the last append call.                                                */
 int32_t hermes_last_launch_count(const hermes_t *h);
 

@@ -22,7 +22,7 @@ HERMES_K_NAMES = ("append", "score_stats", "score_combine", "score_colsum", "sel
 
 EXPORTS = ("hermes_default_config", "hermes_workspace_bytes", "hermes_create", "hermes_append_chunk",
            "hermes_append_chunk_host", "hermes_get_cache", "hermes_len", "hermes_device_status",
-           "hermes_set_profiling", "hermes_get_profile", "hermes_last_score_path",
+           "hermes_set_profiling", "hermes_get_profile", "hermes_last_score_path", "hermes_v_pending",
            "hermes_last_launch_count", "hermes_destroy", "hermes_last_error")
 
 
@@ -82,6 +82,7 @@ def load_library(rebuild_if_stale: bool = True) -> C.CDLL:
     lib.hermes_get_profile.argtypes = [vp, C.POINTER(C.c_float), i32]
     lib.hermes_last_score_path.argtypes = [vp]
     lib.hermes_last_launch_count.argtypes = [vp]
+    lib.hermes_v_pending.argtypes = [vp]
     lib.hermes_destroy.argtypes = [vp]
     lib.hermes_destroy.restype = None
     lib.hermes_last_error.argtypes = [vp]
@@ -243,6 +244,10 @@ def hermes_get_profile(h: Handle) -> dict:
 
 def hermes_last_score_path(h: Handle) -> int:
     return int(load_library().hermes_last_score_path(h.ptr))
+
+
+def hermes_v_pending(h: Handle) -> int:
+    return int(load_library().hermes_v_pending(h.ptr))
 
 
 def hermes_last_launch_count(h: Handle) -> int:

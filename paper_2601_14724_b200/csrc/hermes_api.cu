@@ -61,6 +61,7 @@ extern "C" size_t hermes_workspace_bytes(const hermes_config* c) {
 extern "C" const char* hermes_last_error(const hermes_t* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 extern "C" int32_t hermes_len(const hermes_t* h) { return h ? h->len : 0; }
 extern "C" int32_t hermes_last_score_path(const hermes_t* h) { return h ? h->last_score_path : 0; }
+extern "C" int32_t hermes_v_pending(const hermes_t* h) { return h && h->v_pending ? 1 : 0; }
 extern "C" int32_t hermes_last_launch_count(const hermes_t* h) { return h ? h->last_launches : 0; }
 
 extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t bytes, hermes_t** out) {
@@ -347,7 +348,10 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
   const bool use_tc = evict && g.L > g.n_shallow && h->tc_ok && c.score_path != HERMES_SCORE_SIMT &&
                       (c.score_path == HERMES_SCORE_TCGEN05 || tc_profitable(h, Tn, n_probe));
   h->last_stream = cuda_stream;
-  if (!use_tc) flush_v(h, s);               // no scoring kernel to carry a pending V compaction
+  // a pending V compaction rides in this update's scoring kernel if that kernel is long enough and has the
+  // shared memory for it; otherwise it runs on its own first
+  const bool ride = use_tc && tc_v_ride_ok(h, Tn, n_probe);
+  if (!ride) flush_v(h, s);
   {
     Prof p(h, HERMES_K_APPEND, s);
     const size_t n_vec = size_t(n_new) * row_vecs;
@@ -360,7 +364,7 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
     const float scale_log2 = scale * kLog2e;
     if (g.L > g.n_shallow) {
       if (use_tc) {
-        if (int rc = tc_score(h, Q_probe, Tn, n_probe, scale_log2, s, h->v_pending)) return rc;
+        if (int rc = tc_score(h, Q_probe, Tn, n_probe, scale_log2, s, ride && h->v_pending)) return rc;
         h->v_pending = false;
         h->last_score_path = HERMES_SCORE_TCGEN05;
       } else {
@@ -389,7 +393,7 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
     {
       Prof p(h, HERMES_K_GATHER, s);
       // on the tcgen05 path V stays behind: the next update's scoring kernel compacts it (tc_v_mover), or a flush
-      const bool defer_v = use_tc && c.defer_v != 0;
+      const bool defer_v = ride && c.defer_v != 0;   // the next update will most likely look like this one
       launch_gather(h, defer_v ? kGatherK : kGatherKV, h->cur, s);
       if (defer_v) { h->v_pending = true; h->v_src_buf = h->cur; }
     }

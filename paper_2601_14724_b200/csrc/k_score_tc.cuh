@@ -712,6 +712,23 @@ inline bool tc_profitable(const hermes_t* h, int Tn, int P) {
   return h->geom.G * P >= 32 && Tn >= 512;
 }
 
+// Can a pending V compaction ride in the scoring launch of (Tn, P)?  The mover needs its staging ring beside a
+// K ring of >= 2 stages, and it must finish before the scoring does: one warp per CTA moves ~32 rows per 3 us
+// (one bulk-copy round trip), while the scoring runs at ~2.75e6 exp2 per us on the whole chip (both measured).
+inline bool tc_v_ride_ok(const hermes_t* h, int Tn, int P) {
+  const Geom& g = h->geom;
+  const TcState* st = static_cast<const TcState*>(h->tc_state);
+  const int R = g.G * P;
+  int n_sc = (R + kTcRowsMax - 1) / kTcRowsMax;
+  const int RS = ((R + n_sc - 1) / n_sc + 31) & ~31;
+  const int q_half = (RS + 63) / 64 * 8192;
+  if ((kTcSmemMax - tc_smem_bytes(q_half, 0, true)) / kTcKStage < 2) return false;
+  const double score_us = 2.0 * g.Hq * P * double(Tn) * (g.L - g.n_shallow) * g.B / 2.75e6;
+  const double rows_per_cta = double(g.B) * g.L * g.budget / st->n_sm;
+  const double per = std::min<double>(32.0, double(kTcMoverRing) / double(h->lay.row_bytes));
+  return score_us >= 1.25 * (rows_per_cta / per * 3.0);
+}
+
 struct TcProf {   // same event bracketing as hermes_api.cu's Prof, local to this header
   hermes_t* h; int id; cudaStream_t s;
   TcProf(hermes_t* h_, int id_, cudaStream_t s_) : h(h_), id(id_), s(s_) {

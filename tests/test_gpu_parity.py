@@ -230,19 +230,26 @@ def test_probe_row_ranges_simt_and_tcgen05():
 def test_deferred_v_compaction_equals_immediate():
     """defer_v: V rows moved by the next update's scoring kernel (tc_v_mover) or by a flush must give the same cache,
     bit for bit, as compacting V at once; the summary-token slot and a SIMT-path update in between are covered."""
-    wl = CONFIGS["llava_ov_7b"].scaled(n_layers=7, budget=784, probe_tokens=16)
+    wl = CONFIGS["llava_ov_7b"].scaled(n_layers=7, budget=784, probe_tokens=64)   # long enough scoring for the move to ride
 
     def run(defer, summary):
         ls = LockStep(wl, cfg_over=dict(defer_v=defer, summary_token=summary), oracle_over=dict(summary_token=bool(summary)))
         ls.fill()
+
+        def raw_step(n_probe=None):          # no hermes_get_cache in between (it would flush the pending move)
+            K, V, Q, _ = ls._gen(wl.chunk_tokens, True, n_probe)
+            hb.hermes_append_chunk(ls.h, to_dev(K, wl.dtype), to_dev(V, wl.dtype), to_dev(Q, wl.dtype))
+
         for i in range(5):
-            ls.step(check=False)                                 # deferred moves ride in the next scoring kernel
-        ls.step(check=False, n_probe=2)                          # G*P = 14 < 32: CUDA-core path -> flush before append
-        ls.step(check=False)
+            raw_step()                                           # deferred moves ride in the next scoring kernel
+            assert hb.hermes_v_pending(ls.h) == defer
+        raw_step(n_probe=2)                                      # G*P = 14 < 32: CUDA-core path -> flush before append
+        assert hb.hermes_v_pending(ls.h) == 0
+        raw_step()
         torch.cuda.synchronize()
         out = [{k: t.clone() for k, t in hb.hermes_get_cache(ls.h, 0, l).items() if torch.is_tensor(t)}
                for l in range(wl.n_layers)]                      # get_cache flushes the last pending move
-        assert hb.hermes_device_status(ls.h) == 0
+        assert hb.hermes_v_pending(ls.h) == 0 and hb.hermes_device_status(ls.h) == 0
         ls.close()
         return out
 
