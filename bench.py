@@ -98,7 +98,13 @@ def workload_by_name(name: str):
 
 
 def cfg_index(name: str) -> int:
-    return 3 if name.startswith("sweep") else {"toy": 0, "llava_ov_7b": 1, "qwen25_vl_7b": 2, "batched_72b": 4}[name]
+    return 3 if name.startswith("sweep") else {"toy": 0, "llava_ov_7b": 1, "llava_ov_7b_c16": 1, "qwen25_vl_7b": 2, "batched_72b": 4}[name]
+
+
+def cfg_label(name: str) -> str:
+    if name == "llava_ov_7b_c16":
+        return "SURVEY.md 8(d) row 2b (BASELINE.json configs[1] geometry, the paper's 16-frame chunk)"
+    return f"BASELINE.json configs[{cfg_index(name)}]"
 
 
 def dist_env():
@@ -266,7 +272,7 @@ def run_ours(args):
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "chunk_update_latency_us": ms * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": wl.dtype, "data": "synthetic",
-        "config": {"workload": f"BASELINE.json configs[{cfg_index(wl.name)}] {wl.name}: L{wl.n_layers} Hq{wl.n_q_heads}/Hkv{wl.n_kv_heads} "
+        "config": {"workload": f"{cfg_label(wl.name)} {wl.name}: L{wl.n_layers} Hq{wl.n_q_heads}/Hkv{wl.n_kv_heads} "
                                f"d{wl.head_dim} {wl.dtype}, budget {wl.budget}, chunk {wl.chunk_tokens}, probe {wl.probe_tokens}, "
                                f"T {work['T']}", "streams_per_gpu": B, "parallelism": f"replicas x{world} (independent streams, no collective)",
                    "l2": (f"cache slabs touched per step: {ws_mb:.0f} MB read + {wr_mb:.0f} MB written "

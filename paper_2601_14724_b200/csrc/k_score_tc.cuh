@@ -27,7 +27,12 @@ constexpr int kTcKStage = kTcTile * 256;        // bytes per K tile: 128 tokens 
 constexpr int kTcKStagesMax = 4;                // K ring depth: as many 32 KB stages as fit beside the Q rows
 constexpr int kTcSmemMax = 232448;              // 227 KB dynamic shared memory per CTA
 constexpr int kTcEpiWarps = 16;                 // epilogue warps: 4 per SM sub-partition / TMEM lane quarter
-constexpr int kTcThreads = 64 + kTcEpiWarps * 32 + 32;   // producer, MMA, epilogue, V mover
+constexpr int kTcCtlWarps = 4;                  // warpgroup 0: producer, MMA issuer, V mover, (idle)
+constexpr int kTcThreads = (kTcCtlWarps + kTcEpiWarps) * 32;   // the epilogue warps are warpgroups 1-4
+constexpr int kTcRegsLaunch = 96;                // registers per thread at launch (640 threads)
+constexpr int kTcRegsCtl = 64, kTcRegsEpi = 104; // setmaxnreg: warpgroup 0 releases registers, the epilogue warps take them
+// setmaxnreg.inc draws only on registers released by setmaxnreg.dec in the same CTA -- it spins forever otherwise
+static_assert((kTcRegsLaunch - kTcRegsCtl) * kTcCtlWarps >= (kTcRegsEpi - kTcRegsLaunch) * kTcEpiWarps, "register pool");
 constexpr int kTcMoverRing = 32768;             // shared-memory staging of the V mover
 constexpr int kTcSegTiles = 4;                  // pass 1: 128-token tiles per segment (one partial pair per
                                                 // segment, so the merge order never depends on the CTA schedule)
@@ -185,7 +190,7 @@ __device__ inline void tc_producer(const TcSmem& s, const TcBars& b, const CUten
 // A TMEM stage (256 columns) holds a "half-group" = 2 row blocks x 128 tokens; epilogue warp
 // (row block rbl, 64-token half th, lane quarter lg) takes its 64 columns as two 32-column blocks.
 // =====================================================================================================
-template <int kVar, bool kTrace>
+template <int kVar, bool kTrace, bool kEpi>
 __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const CUtensorMap* tmap_q, const CUtensorMap* tmap_k,
                                          const TcArgs& a, uint32_t tmem_base, TcRole& st) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -193,9 +198,9 @@ __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const
   const int s0 = tc_unit_begin(U, gridDim.x, blockIdx.x), s1 = tc_unit_begin(U, gridDim.x, blockIdx.x + 1);
   long long* const trace_p = a.trace;
 
-  if (warp == 0) {
+  if (!kEpi && warp == 0) {
     if (lane == 0) tc_producer<true, kTrace>(s, b, tmap_q, tmap_k, a, s0, s1, st, trace_p);
-  } else if (warp == 1) {
+  } else if (!kEpi && warp == 1) {
     // ---------------- MMA issuer: the whole warp runs the loop, one elected lane issues ----------------
     const uint32_t idesc = ptx::idesc_bf16_f32(128, kTcTile);
     const uint32_t q_lo = ptx::smem_desc_lo(ptx::smem_u32(s.q)), k_lo = ptx::smem_desc_lo(ptx::smem_u32(s.k));
@@ -251,9 +256,9 @@ __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const
       if (++x == a.spg) { x = 0; g.next(a); new_group = true; }
     }
     st.ks = ks; st.kph = kph; st.as = as; st.aph = aph; st.n_q = n_q;
-  } else if (warp < 2 + kTcEpiWarps) {
+  } else if (kEpi) {
     // ---------------- epilogue: one probe row x 64 tokens per thread per stage ----------------
-    const int e = warp - 2, rbl = e >> 3, th = (e >> 2) & 1, lg = warp & 3;
+    const int e = warp - kTcCtlWarps, rbl = e >> 3, th = (e >> 2) & 1, lg = warp & 3;
     const uint32_t t_addr = tmem_base + (uint32_t(lg * 32) << 16) + rbl * kTcTile + th * 64;
     int as = st.as, aph = st.aph, trace_n = 0;
     const int trole = e == 0 ? 2 : 3;
@@ -409,7 +414,7 @@ __device__ __noinline__ void tc_merge_rows(const float2* pr, int n_slot, int row
 // holds a chunk of <= 256 probe rows of the 128-token tile; epilogue warp (lane quarter lg, column
 // quarter cq) takes 32-column blocks cq and cq + 4 of the chunk.
 // =====================================================================================================
-template <int kVar, bool kTrace>
+template <int kVar, bool kTrace, bool kEpi>
 __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const CUtensorMap* tmap_q, const CUtensorMap* tmap_k,
                                          const TcArgs& a, uint32_t tmem_base, TcRole& st) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -417,9 +422,9 @@ __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const
   const int u0 = tc_unit_begin(U, gridDim.x, blockIdx.x), u1 = tc_unit_begin(U, gridDim.x, blockIdx.x + 1);
   long long* const trace_p = a.trace ? a.trace + kTcTraceStride : nullptr;
 
-  if (warp == 0) {
+  if (!kEpi && warp == 0) {
     if (lane == 0) tc_producer<false, kTrace>(s, b, tmap_q, tmap_k, a, u0, u1, st, trace_p);
-  } else if (warp == 1) {
+  } else if (!kEpi && warp == 1) {
     // ---------------- MMA issuer: the whole warp runs the loop, one elected lane issues ----------------
     const uint32_t q_lo = ptx::smem_desc_lo(ptx::smem_u32(s.q)), k_lo = ptx::smem_desc_lo(ptx::smem_u32(s.k));
     const uint32_t q_half16 = uint32_t(a.q_half_bytes) >> 4;
@@ -460,9 +465,9 @@ __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const
       if (++ks == a.n_kst) { ks = 0; kph ^= 1; }
       if (++t == a.tpg) { t = 0; g.next(a); new_group = true; }
     }
-  } else if (warp < 2 + kTcEpiWarps) {
+  } else if (kEpi) {
     // ---------------- epilogue: one token per thread; warp (lane quarter lg, column quarter cq) ----------------
-    const int e = warp - 2, cq = e >> 2, lg = warp & 3;
+    const int e = warp - kTcCtlWarps, cq = e >> 2, lg = warp & 3;
     const int tok_in_tile = lg * 32 + lane;
     const uint32_t t_addr = tmem_base + (uint32_t(lg * 32) << 16) + cq * 32;
     int as = st.as, aph = st.aph, trace_n = 0;
@@ -516,7 +521,7 @@ __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const
         if (tr) TC_TRACE(trole, 5);
         const int bl = g.bl(a), rows_total = a.g.Hq * a.g.p_max;
         tc_merge_rows(reinterpret_cast<const float2*>(a.g.partial) + size_t(bl) * a.spg * rows_total + g.stat_row0(a),
-                      a.spg, rows_total, g.rs_valid(a), s.c, threadIdx.x - 64, g.sc * a.RS, a.P,
+                      a.spg, rows_total, g.rs_valid(a), s.c, threadIdx.x - kTcCtlWarps * 32, g.sc * a.RS, a.P,
                       g.ls >= a.g.L - a.g.n_shallow - a.g.n_deep ? a.g.probe_deep_begin : 0);
         ptx::named_bar_sync(1, kTcEpiWarps * 32);
         if (tr) TC_TRACE(trole, 6);
@@ -556,7 +561,7 @@ __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const
   }
 }
 
-// V mover (warp 2 + kTcEpiWarps): compaction of V needs no arithmetic and nothing in the scoring of the NEXT update
+// V mover (warp 2): compaction of V needs no arithmetic and nothing in the scoring of the NEXT update
 // reads V, so k_gather leaves V behind and this warp moves the kept rows V[kept[s]] -> V'[s] of the previous update
 // with 1D bulk copies (global -> shared -> global) while the tensor / XU pipes score: one row per lane, one
 // mbarrier wait per batch.  The CTA's share is ~1200 rows of 1 KB over ~200 us: a few GB/s per SM.
@@ -609,12 +614,23 @@ k_tc_score(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ C
   const uint32_t tmem_base = tc_prologue(s, b, a, &tmap_q, &tmap_k);
   pdl_wait();                       // the chunk's K rows come from k_append
   if (threadIdx.x == 0) pdl_launch_dependents();
-  if ((threadIdx.x >> 5) == 2 + kTcEpiWarps && a.v_base != nullptr) tc_v_mover(s, b, a);
+  // 20 warps start with 96 registers each; warpgroup 0 hands 32 of them to the 16 epilogue warps (+8 each).  Each side stays in
+  // its own branch until the end of the kernel (ptxas bounds registers per region between setmaxnreg and the join).
   TcRole st;
-  tc_pass1<kVar, kTrace>(s, b, &tmap_q, &tmap_k, a, tmem_base, st);
-  if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.trace[4 * kTcTraceN + 2 * blockIdx.x + 1] = t; }
-  if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.trace[kTcTraceStride + 4 * kTcTraceN + 2 * blockIdx.x] = t; }
-  tc_pass2<kVar, kTrace>(s, b, &tmap_q, &tmap_k, a, tmem_base, st);
+  if ((threadIdx.x >> 5) < kTcCtlWarps) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kTcRegsCtl));
+    if ((threadIdx.x >> 5) == 2 && a.v_base != nullptr) tc_v_mover(s, b, a);
+    tc_pass1<kVar, kTrace, false>(s, b, &tmap_q, &tmap_k, a, tmem_base, st);
+    if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) {
+      long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+      a.trace[4 * kTcTraceN + 2 * blockIdx.x + 1] = t; a.trace[kTcTraceStride + 4 * kTcTraceN + 2 * blockIdx.x] = t;
+    }
+    tc_pass2<kVar, kTrace, false>(s, b, &tmap_q, &tmap_k, a, tmem_base, st);
+  } else {
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kTcRegsEpi));
+    tc_pass1<kVar, kTrace, true>(s, b, &tmap_q, &tmap_k, a, tmem_base, st);
+    tc_pass2<kVar, kTrace, true>(s, b, &tmap_q, &tmap_k, a, tmem_base, st);
+  }
   ptx::tc_fence_before();
   __syncthreads();
   if (kTrace && a.trace != nullptr && threadIdx.x == 0 && blockIdx.x < 256) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.trace[kTcTraceStride + 4 * kTcTraceN + 2 * blockIdx.x + 1] = t; }

@@ -60,6 +60,16 @@ def test_llava_ov_7b_full_size():
     ls.close()
 
 
+def test_llava_ov_7b_16_frame_chunk_full_size():
+    """the paper's 16-frame chunk (3136 tokens) at configs[1] geometry --
+    every update evicts a third of the cache; T = 9408 = 73.5 token tiles."""
+    wl = CONFIGS["llava_ov_7b_c16"]
+    ls, reps = _run(wl, 2, n_warm=1)
+    assert all(r["T"] == 9408 for r in reps)
+    assert hb.hermes_last_score_path(ls.h) == hb.HERMES_SCORE_TCGEN05
+    ls.close()
+
+
 def test_qwen25_vl_mrope_reduced_and_all_axes():
     wl = CONFIGS["qwen25_vl_7b"].scaled(n_layers=6, budget=1024, probe_tokens=32, pos_offset=5)
     ls, reps = _run(wl, 3, n_warm=1)

@@ -119,6 +119,8 @@ CONFIGS = {
                     drift_beta=0.0, apply_rope=True, timed_updates=10),
     # configs[1]: LLaVA-OV-7B geometry (Qwen2-7B backbone), the benchmark workload
     "llava_ov_7b": _llava("llava_ov_7b"),
+    # the same geometry with the paper's 16-frame chunk (16 frames x 196 tokens)
+    "llava_ov_7b_c16": _llava("llava_ov_7b_c16", seed=2016).scaled(chunk_tokens=3136, timed_updates=64),
     # configs[2]: Qwen2.5-VL-7B geometry, M-RoPE, 64 tokens per temporal step, t-only compaction
     "qwen25_vl_7b": Workload(name="qwen25_vl_7b", n_layers=28, n_q_heads=28, n_kv_heads=4,
                              head_dim=128, dtype="bf16", tokens_per_frame=64, budget=8192,
