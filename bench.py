@@ -159,6 +159,8 @@ def run_ours(args):
         over.update(reindex_mode=hb.HERMES_REINDEX_LAZY, max_position=args.max_position)
     if args.summary_token:
         over.update(summary_token=1)
+    if args.no_defer_v:
+        over.update(defer_v=0)
     cfg = hb.config_for_workload(wl, device=local_rank, **over)
     h = hb.hermes_create(cfg)
 
@@ -351,6 +353,7 @@ def main():
     ap.add_argument("--max-position", type=int, default=32768, help="lazy re-indexing: the model's position limit")
     ap.add_argument("--summary-token", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-defer-v", action="store_true", help="compact V in the gather kernel instead of inside the next scoring launch")
     args = ap.parse_args()
     if args.impl == "reference":
         out = run_reference(args)
