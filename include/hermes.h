@@ -135,9 +135,12 @@ int hermes_create(const hermes_config *cfg, void *workspace, size_t bytes, herme
 int hermes_append_chunk(hermes_t *h, const void *K_new, const void *V_new, const void *Q_probe,
                         int32_t n_new, int32_t n_probe, int32_t pos_start, void *cuda_stream);
 
-/* Same update with HOST buffers (pinned memory recommended): stages K_new/V_new/Q_probe to the device
- * with cudaMemcpyAsync on `cuda_stream`, runs the update, and, if kept_out != NULL, copies the kept
- * index lists I_l [B, L, budget] int32 back to the host (only meaningful when an eviction ran).        */
+/* Same update with HOST buffers (pinned memory recommended): stages Q_probe and K_new to the device with
+ * cudaMemcpyAsync on `cuda_stream`, V_new on a library-owned side stream (created on first use) so that its
+ * copy overlaps the scoring kernels, which never read V; the V rows are appended behind an event wait on
+ * `cuda_stream`, so everything the call enqueues is ordered on `cuda_stream` when it returns.  If
+ * kept_out != NULL, copies the kept index lists I_l [B, L, budget] int32 back to the host (only meaningful
+ * when an eviction ran).  The host buffers must stay valid until `cuda_stream` has passed the call.          */
 int hermes_append_chunk_host(hermes_t *h, const void *K_new_host, const void *V_new_host,
                              const void *Q_probe_host, int32_t n_new, int32_t n_probe,
                              int32_t pos_start, int32_t *kept_out_host, void *cuda_stream);

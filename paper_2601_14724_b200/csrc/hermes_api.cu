@@ -180,6 +180,7 @@ extern "C" void hermes_destroy(hermes_t* h) {
   if (!h) return;
   if (h->timer.created)
     for (int i = 0; i < HERMES_K_COUNT; ++i) { cudaEventDestroy(h->timer.beg[i]); cudaEventDestroy(h->timer.end[i]); }
+  if (h->side_stream) { cudaStreamSynchronize(h->side_stream); cudaStreamDestroy(h->side_stream); cudaEventDestroy(h->ev_k_done); cudaEventDestroy(h->ev_v_done); }
   tc_destroy(h);
   delete h;
 }
@@ -307,8 +308,10 @@ void flush_v(hermes_t* h, cudaStream_t s) {
 }
 }  // namespace
 
-extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V_new, const void* Q_probe,
-                                   int32_t n_new, int32_t n_probe, int32_t pos_start, void* cuda_stream) {
+// v_ready != NULL (host entry point): V_new is still being copied on another stream; its rows are appended by a second
+// k_append launch once the scoring kernels are enqueued, behind a wait on that event.
+static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const void* Q_probe,
+                       int32_t n_new, int32_t n_probe, int32_t pos_start, void* cuda_stream, cudaEvent_t v_ready) {
   if (!h) return HERMES_EINVAL;
   const hermes_config& c = h->cfg;
   Geom& g = h->geom;
@@ -357,8 +360,18 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
     const size_t n_vec = size_t(n_new) * row_vecs;
     const int gx = int(std::min<size_t>((n_vec + 511) / 512, 64));
     launch_pdl(k_append, dim3(std::max(gx, 1), BL), dim3(256), 0, s, g, static_cast<const uint4*>(K_new), static_cast<const uint4*>(V_new),
-               h->cur, h->len, n_new, row_vecs, int(p0));
+               h->cur, h->len, n_new, row_vecs, int(p0), v_ready ? kAppendK : (kAppendK | kAppendV));
   }
+  auto append_v_late = [&]() {                       // nothing before the gather (or a later reader) needs V_new
+    if (!v_ready) return;
+    cudaStreamWaitEvent(s, v_ready, 0);
+    const size_t n_vec = size_t(n_new) * row_vecs;
+    const int gx = int(std::min<size_t>((n_vec + 511) / 512, 64));
+    launch_pdl(k_append, dim3(std::max(gx, 1), BL), dim3(256), 0, s, g, static_cast<const uint4*>(K_new), static_cast<const uint4*>(V_new),
+               h->cur, h->len, n_new, row_vecs, int(p0), kAppendV);
+    ++h->last_launches;
+  };
+  if (!evict) append_v_late();
   if (evict) {
     const float scale = c.softmax_scale > 0.f ? c.softmax_scale : float(1.0 / std::sqrt(double(c.head_dim)));
     const float scale_log2 = scale * kLog2e;
@@ -374,6 +387,7 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
         h->n_vh = g.Hkv;
       }
     }
+    append_v_late();
     {
       Prof p(h, HERMES_K_SELECT, s);
       if (g.L > g.n_shallow) ++h->last_launches;
@@ -415,6 +429,11 @@ extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V
   return HERMES_OK;
 }
 
+extern "C" int hermes_append_chunk(hermes_t* h, const void* K_new, const void* V_new, const void* Q_probe,
+                                   int32_t n_new, int32_t n_probe, int32_t pos_start, void* cuda_stream) {
+  return append_impl(h, K_new, V_new, Q_probe, n_new, n_probe, pos_start, cuda_stream, nullptr);
+}
+
 extern "C" int hermes_append_chunk_host(hermes_t* h, const void* K_host, const void* V_host, const void* Q_host,
                                         int32_t n_new, int32_t n_probe, int32_t pos_start,
                                         int32_t* kept_out_host, void* cuda_stream) {
@@ -427,12 +446,26 @@ extern "C" int hermes_append_chunk_host(hermes_t* h, const void* K_host, const v
   const size_t BL = size_t(c.n_streams) * c.n_layers;
   const size_t kv_bytes = BL * n_new * h->lay.row_bytes;
   char* sk = h->ws + h->lay.stage_k; char* sv = h->ws + h->lay.stage_v; char* sq = h->ws + h->lay.stage_q;
-  CUDA_TRY(h, cudaMemcpyAsync(sk, K_host, kv_bytes, cudaMemcpyHostToDevice, s));
-  CUDA_TRY(h, cudaMemcpyAsync(sv, V_host, kv_bytes, cudaMemcpyHostToDevice, s));
+  // Q and K go first on the caller's stream; V follows on a side stream once K is across, so that it moves while
+  // the scoring kernels (which never read V) run.  The event after the K copy also orders the side stream behind
+  // every earlier reader of the V staging buffer.
+  if (!h->side_stream) {
+    CUDA_TRY(h, cudaStreamCreateWithFlags(&h->side_stream, cudaStreamNonBlocking));
+    CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_k_done, cudaEventDisableTiming));
+    CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_v_done, cudaEventDisableTiming));
+  }
   if (Q_host) CUDA_TRY(h, cudaMemcpyAsync(sq, Q_host, BL * c.n_q_heads * n_probe * c.head_dim * h->lay.esize, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(h, cudaMemcpyAsync(sk, K_host, kv_bytes, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(h, cudaEventRecord(h->ev_k_done, s));
+  CUDA_TRY(h, cudaStreamWaitEvent(h->side_stream, h->ev_k_done, 0));
+  CUDA_TRY(h, cudaMemcpyAsync(sv, V_host, kv_bytes, cudaMemcpyHostToDevice, h->side_stream));
+  CUDA_TRY(h, cudaEventRecord(h->ev_v_done, h->side_stream));
   const int len_before = h->len;
-  int rc = hermes_append_chunk(h, sk, sv, Q_host ? sq : nullptr, n_new, n_probe, pos_start, cuda_stream);
-  if (rc != HERMES_OK) return rc;
+  int rc = append_impl(h, sk, sv, Q_host ? sq : nullptr, n_new, n_probe, pos_start, cuda_stream, h->ev_v_done);
+  if (rc != HERMES_OK) {                               // nothing was enqueued: still join the side stream
+    cudaStreamWaitEvent(s, h->ev_v_done, 0);
+    return rc;
+  }
   const bool evicted = Q_host && len_before + n_new > c.budget;
   if (kept_out_host && evicted)
     CUDA_TRY(h, cudaMemcpyAsync(kept_out_host, h->geom.kept, BL * c.budget * 4, cudaMemcpyDeviceToHost, s));

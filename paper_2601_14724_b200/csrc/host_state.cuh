@@ -158,6 +158,8 @@ struct hermes {
   int last_score_path = 0;
   int last_launches = 0;
   int n_sm = 148;
+  cudaStream_t side_stream = nullptr;   // host entry point: V's host-to-device copy (created on first use)
+  cudaEvent_t ev_k_done = nullptr, ev_v_done = nullptr;
   int n_vh = 0;             // column-sum slots written by the last scoring pass
   // deferred V compaction: after an eviction on the tcgen05 path k_gather moves only K; the kept V rows still sit
   // in buffer v_src_buf and are moved into the current buffer by the NEXT update's scoring kernel (or by a flush)

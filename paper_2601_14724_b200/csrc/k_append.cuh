@@ -6,14 +6,17 @@
 namespace hk {
 
 // K_new/V_new: [B*L][n_new][row_elems]; destination rows [len, len+n_new) of the current buffer.
-// row_vecs = 16-byte vectors per token row.
+// row_vecs = 16-byte vectors per token row.  what: bit 0 = K rows + positions + wmax reset, bit 1 = V rows (the host
+// entry point appends V in a second launch, after scoring, so that V's host-to-device copy overlaps the scoring).
+constexpr int kAppendK = 1, kAppendV = 2;
 __global__ void __launch_bounds__(256)
 k_append(Geom g, const uint4* __restrict__ k_new, const uint4* __restrict__ v_new,
-         int cur, int len, int n_new, int row_vecs, int pos_start) {
+         int cur, int len, int n_new, int row_vecs, int pos_start, int what) {
   pdl_wait();
   pdl_launch_dependents();
   const int bl = blockIdx.y;                        // b * L + l
-  if (blockIdx.x == 0 && threadIdx.x == 0) g.wmax[bl] = 0u;   // reset the per-layer max of W for this step
+  const bool do_k = what & kAppendK, do_v = what & kAppendV;
+  if (do_k && blockIdx.x == 0 && threadIdx.x == 0) g.wmax[bl] = 0u;   // reset the per-layer max of W for this step
   const size_t slab = size_t(bl) * 2 + cur;
   const size_t n_vec = size_t(n_new) * row_vecs;
   const uint4* ks = k_new + size_t(bl) * n_vec;
@@ -23,12 +26,23 @@ k_append(Geom g, const uint4* __restrict__ k_new, const uint4* __restrict__ v_ne
   const size_t stride = size_t(gridDim.x) * blockDim.x;
   size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x;
   // 2 independent (K,V) pairs in flight per thread
-  for (; i + stride < n_vec; i += 2 * stride) {
-    uint4 a = ldg_stream(ks + i), b = ldg_stream(vs + i);
-    uint4 c = ldg_stream(ks + i + stride), d = ldg_stream(vs + i + stride);
-    kd[i] = a; vd[i] = b; kd[i + stride] = c; vd[i + stride] = d;
+  if (do_k && do_v) {
+    for (; i + stride < n_vec; i += 2 * stride) {
+      uint4 a = ldg_stream(ks + i), b = ldg_stream(vs + i);
+      uint4 c = ldg_stream(ks + i + stride), d = ldg_stream(vs + i + stride);
+      kd[i] = a; vd[i] = b; kd[i + stride] = c; vd[i + stride] = d;
+    }
+    if (i < n_vec) { kd[i] = ldg_stream(ks + i); vd[i] = ldg_stream(vs + i); }
+  } else {
+    const uint4* src = do_k ? ks : vs;
+    uint4* dst = do_k ? kd : vd;
+    for (; i + stride < n_vec; i += 2 * stride) {
+      uint4 a = ldg_stream(src + i), c = ldg_stream(src + i + stride);
+      dst[i] = a; dst[i + stride] = c;
+    }
+    if (i < n_vec) dst[i] = ldg_stream(src + i);
   }
-  if (i < n_vec) { kd[i] = ldg_stream(ks + i); vd[i] = ldg_stream(vs + i); }
+  if (!do_k) return;
 
   // arrival positions, identical across layers (1D: pos_start + j; M-RoPE: (t0 + j/tpt, grid row, grid col))
   int32_t* pos = g.posc + slab * g.n_axes * g.cap;
