@@ -187,6 +187,42 @@ def test_determinism_and_host_api():
         assert torch.equal(kept[0, l].cuda(), a[l]["last_kept"])
 
 
+def test_host_entry_point_fill_and_batched_streams():
+    """Host-buffer entry point on the paths the test above does not reach: appends without a probe (no eviction:
+    the V rows arrive through the late, V-only append) and B > 1 streams; caches must equal the device entry point's."""
+    wl = CONFIGS["batched_72b"].scaled(n_layers=4, n_streams=2, budget=392, probe_tokens=8)
+    from workloads import chunk_kv, probe_q
+    pool = []
+    for u in range(4):                                   # two fills, then two evicting updates
+        per = [chunk_kv(wl, b, u, u * wl.chunk_tokens, wl.chunk_tokens) for b in range(wl.n_streams)]
+        K = np.stack([p[0] for p in per]); V = np.stack([p[1] for p in per])
+        Q = np.stack([probe_q(wl, b, u) for b in range(wl.n_streams)]) if u >= 2 else None
+        pool.append((K, V, Q))
+
+    def run(host: bool):
+        h = hb.hermes_create(hb.config_for_workload(wl))
+        for K, V, Q in pool:
+            if host:
+                args = [None if x is None else torch.from_numpy(x).to(torch.bfloat16).pin_memory() for x in (K, V, Q)]
+                hb.hermes_append_chunk_host(h, *args)
+            else:
+                hb.hermes_append_chunk(h, to_dev(K, "bf16"), to_dev(V, "bf16"), None if Q is None else to_dev(Q, "bf16"))
+            torch.cuda.synchronize()
+        out = [[{k: t.clone() for k, t in hb.hermes_get_cache(h, b, l).items() if torch.is_tensor(t)}
+                for l in range(wl.n_layers)] for b in range(wl.n_streams)]
+        n = hb.hermes_len(h)
+        hb.hermes_destroy(h)
+        return out, n
+
+    a, na = run(False)
+    b, nb = run(True)
+    assert na == nb == wl.budget
+    for s in range(wl.n_streams):
+        for l in range(wl.n_layers):
+            for key in ("k", "v", "pos", "last_kept"):
+                assert torch.equal(a[s][l][key], b[s][l][key]), (s, l, key)
+
+
 def test_lazy_reindexing_toy_and_bf16():
     """DESIGN f2 (PAPER.md:126-128): lazy mode copies kept keys bit for bit and keeps their original indices;
     the step after which the next chunk would cross max_position re-indexes exactly like the eager path."""
