@@ -266,9 +266,13 @@ def run_ours(args):
     roof["peak_source"] = ("derived: 16 exp2/clk/SM x 148 SMs x clocks.max.sm (DESIGN.md section 6)" if roof["bound"] == "alu"
                            else pk["source"])
     t_roof = max(work["bytes_min"] / (pk["hbm"] * 1e9), work["flops"] / (pk["tensor"] * 1e12))
+    # third floor, not part of north_star's roofline but the binding one on the tcgen05 path: the two-pass softmax column
+    # sum needs 2 exp2 per (probe row, token) at 16 / clk / SM
+    exp2_floor = (2.0 * work["flops"] / (2.0 * wl.head_dim)) / (16 * 148 * ((clocks or {}).get("sm_max_mhz") or 1965.0) * 1e6)
     step_roof = dict(bound="hbm" if work["bytes_min"] / (pk["hbm"] * 1e9) >= work["flops"] / (pk["tensor"] * 1e12) else "tensor",
                      roofline_us=t_roof * 1e6, measured_us=ms * 1e3, frac=t_roof / (ms * 1e-3),
-                     bytes_min=work["bytes_min"], flops=work["flops"])
+                     bytes_min=work["bytes_min"], flops=work["flops"],
+                     exp2_floor_us=exp2_floor * 1e6 if score_path == "tcgen05" else None)
     out = {
         "metric": METRIC, "value": job_value(wl, world, B, ms), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "chunk_update_latency_us": ms * 1e3,
