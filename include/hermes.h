@@ -60,7 +60,8 @@ typedef struct {
   int32_t n_streams;            /* B independent streams advanced by every call                */
   int32_t tokens_per_frame;     /* N_f; informational                                          */
   int32_t budget;               /* |M| tokens kept per layer                    */
-  int32_t max_chunk_tokens;     /* largest n_new                                               */
+  int32_t max_chunk_tokens;     /* largest n_new (binding for the host entry point and for LAZY re-indexing; an
+                                   append through hermes_append_chunk is otherwise bounded by max_tokens only) */
   int32_t max_tokens;           /* slots per layer; 0 -> budget + max_chunk_tokens             */
   int32_t max_probe_tokens;     /* largest n_probe                                             */
   int32_t n_shallow, n_deep;    /* -1 -> max(1, round(0.1 L)), max(1, round(0.3 L)) */
@@ -92,6 +93,10 @@ typedef struct {
                                    kept V rows to be moved by the NEXT update's scoring kernel (V is not read by
                                    scoring, so the copy hides behind it); hermes_get_cache() and updates that do
                                    not score on tcgen05 first run the pending move on their own.  0: never defer */
+  int32_t defer_k;              /* 1 (default, needs defer_v): the same for K.  The kept K rows of the slabs the next
+                                   scoring launch reaches late are compacted and re-rotated by that launch's mover
+                                   warps (which deliver each slab before its keys are loaded); only the first slabs of
+                                   the schedule are compacted at once.  0: K is always compacted at once            */
   int32_t score_path;           /* HERMES_SCORE_*: AUTO picks tcgen05 when the contraction is dense */
   int32_t device;               /* CUDA device ordinal                                         */
 } hermes_config;
@@ -145,8 +150,8 @@ int hermes_append_chunk_host(hermes_t *h, const void *K_new_host, const void *V_
                              const void *Q_probe_host, int32_t n_new, int32_t n_probe,
                              int32_t pos_start, int32_t *kept_out_host, void *cuda_stream);
 
-/* Fills *out for (stream, layer).  No synchronisation; if a V compaction is pending (defer_v) it is enqueued
- * on the stream of the last append first.                                                              */
+/* Fills *out for (stream, layer).  No synchronisation; if a compaction is pending (defer_v / defer_k) it is
+ * enqueued on the stream of the last append first.                                                     */
 int hermes_get_cache(hermes_t *h, int32_t stream, int32_t layer, hermes_cache_view *out);
 
 /* Host-tracked token count per layer (same for every stream and layer).                              */
@@ -169,6 +174,9 @@ int32_t hermes_last_score_path(const hermes_t *h);
 
 /* 1 if a V compaction is pending (defer_v): the kept V rows of the last eviction have not been moved yet.        */
 int32_t hermes_v_pending(const hermes_t *h);
+
+/* Number of (stream, layer) slabs whose K compaction is pending (defer_k); 0 if none.                             */
+int32_t hermes_k_pending(const hermes_t *h);
 
 /* Number of kernels launched by the last append call.                                                */
 int32_t hermes_last_launch_count(const hermes_t *h);

@@ -77,7 +77,9 @@ class LockStep:
         Q = np.stack([p[2] for p in per]) if with_probe else None
         return K, V, Q, [p[3] for p in per]
 
-    def _after(self, n_new, new_ids, evicted, p0=0):
+    def _after(self, n_new, new_ids, evicted, p0=0, track_ids=True):
+        """Host-side mirrors of the library's position counters; with track_ids also the token ids of the kept
+        slots (that part calls hermes_get_cache, which flushes a pending compaction)."""
         span = n_new
         if self.ocfg.rope_mode == "m3d":
             tpt = self.ocfg.mrope_grid_h * self.ocfg.mrope_grid_w
@@ -87,6 +89,8 @@ class LockStep:
         self.next_pos = p0 + span
         if evicted and (c.reindex_mode == "eager" or ho.lazy_reindex_due(c, p0 + span)):
             self.next_pos = c.pos_offset + (c.budget if c.rope_mode == "1d" else min(self.t_steps_seen, c.budget))
+        if not track_ids:
+            return
         for b in range(self.B):
             self.ids[b] = np.concatenate([self.ids[b], np.broadcast_to(new_ids[b], (self.wl.n_layers, n_new))], 1)
         if evicted:
@@ -103,6 +107,17 @@ class LockStep:
             K, V, _, ids = self._gen(n, False)
             hb.hermes_append_chunk(self.h, to_dev(K, self.wl.dtype), to_dev(V, self.wl.dtype), None)
             self._after(n, ids, False, p0)
+
+    def raw_step(self, n_new=None, n_probe=None):
+        """One evicting update with nothing but hermes_append_chunk on the library side (no hermes_get_cache: a
+        pending compaction stays pending and rides in the next scoring launch)."""
+        wl = self.wl
+        n_new = wl.chunk_tokens if n_new is None else n_new
+        p0 = int(self._arrival(n_new)[0, 0])
+        K, V, Q, ids = self._gen(n_new, True, n_probe)
+        T = hb.hermes_len(self.h) + n_new
+        hb.hermes_append_chunk(self.h, to_dev(K, wl.dtype), to_dev(V, wl.dtype), to_dev(Q, wl.dtype))
+        self._after(n_new, ids, T > wl.budget, p0, track_ids=False)
 
     def step(self, check=True, n_new=None, n_probe=None, pos_start=-1):
         wl = self.wl

@@ -53,11 +53,66 @@ def test_llava_geometry_reduced_multi_tile_ragged():
 
 
 def test_llava_ov_7b_full_size():
-    """configs[1] at full size, in the launch configuration bench.py times: 2 lock-step updates."""
+    """configs[1] at full size, 2 lock-step updates.  Every checked update starts from a flushed cache
+    (hermes_get_cache runs a pending compaction), so the scoring launch here carries no movers; the launch
+    bench.py times is checked by test_timed_launch_configuration_full_size."""
     wl = CONFIGS["llava_ov_7b"]
     ls, reps = _run(wl, 2, n_warm=2)
     assert all(r["T"] == 6468 for r in reps)
     ls.close()
+
+
+def _raw_steps_vs_lockstep(wl, n_steps, over=None, oover=None):
+    """The launch configuration bench.py times: `n_steps` consecutive evicting updates through hermes_append_chunk
+    with NO hermes_get_cache in between, so that the previous update's K and V compaction rides in every scoring
+    launch (mover warps, 2-stage K ring, ramped batch schedule).  The final cache must equal, bit for bit, the cache
+    of a handle that never defers (defer_v = defer_k = 0) and is compared with the oracle, lock-step, at every step
+    on the same inputs."""
+    over, oover = dict(over or {}), dict(oover or {})
+    a = LockStep(wl, cfg_over=over, oracle_over=oover)
+    a.fill()
+    pend = []
+    for _ in range(n_steps):
+        a.raw_step()
+        pend.append((hb.hermes_v_pending(a.h), hb.hermes_k_pending(a.h)))
+    torch.cuda.synchronize()
+    assert hb.hermes_last_score_path(a.h) == hb.HERMES_SCORE_TCGEN05
+    got = [[{k: t.clone() for k, t in hb.hermes_get_cache(a.h, b, l).items() if torch.is_tensor(t)}
+            for l in range(wl.n_layers)] for b in range(wl.n_streams)]
+    assert hb.hermes_v_pending(a.h) == 0 and hb.hermes_k_pending(a.h) == 0 and hb.hermes_device_status(a.h) == 0
+    a.close()
+    ref = LockStep(wl, cfg_over=dict(over, defer_v=0, defer_k=0), oracle_over=oover)
+    ref.fill()
+    for _ in range(n_steps):
+        ref.step(check=True)
+    for b in range(wl.n_streams):
+        for l in range(wl.n_layers):
+            v = hb.hermes_get_cache(ref.h, b, l)
+            for key in ("k", "v", "pos", "last_kept", "last_scores"):
+                assert torch.equal(v[key], got[b][l][key]), (b, l, key)
+    ref.close()
+    return pend
+
+
+def test_timed_launch_configuration_full_size():
+    """configs[1] at full size exactly as bench.py runs it: 5 back-to-back evicting updates, movers riding."""
+    pend = _raw_steps_vs_lockstep(CONFIGS["llava_ov_7b"], 5)
+    assert all(v == 1 for v, _ in pend)                    # V always rides in the next scoring launch
+    assert all(k > 0 for _, k in pend)                     # and so does K of most slabs
+
+
+def test_timed_launch_configuration_reduced_variants():
+    """Same protocol on reduced geometries: M-RoPE (three delta axes), the summary token slot, lazy re-indexing
+    (pure copies), a chunk that is not a multiple of anything, and B > 1 streams."""
+    _raw_steps_vs_lockstep(CONFIGS["llava_ov_7b"].scaled(n_layers=7, budget=784, probe_tokens=64), 4)
+    _raw_steps_vs_lockstep(CONFIGS["llava_ov_7b"].scaled(n_layers=7, budget=784, probe_tokens=64), 3,
+                           over=dict(summary_token=1), oover=dict(summary_token=True))
+    _raw_steps_vs_lockstep(CONFIGS["qwen25_vl_7b"].scaled(n_layers=6, budget=1024, probe_tokens=64, pos_offset=5), 3)
+    _raw_steps_vs_lockstep(CONFIGS["batched_72b"].scaled(n_layers=5, n_streams=3, budget=1177, probe_tokens=48), 3)
+    wl = CONFIGS["llava_ov_7b"].scaled(n_layers=6, budget=784, probe_tokens=64)
+    mp = 784 + 196 * 4                                      # the 3rd update re-indexes, the others copy
+    _raw_steps_vs_lockstep(wl, 5, over=dict(reindex_mode=hb.HERMES_REINDEX_LAZY, max_position=mp),
+                           oover=dict(reindex_mode="lazy", max_position=mp, max_chunk_span=wl.chunk_tokens))
 
 
 def test_llava_ov_7b_16_frame_chunk_full_size():
@@ -279,7 +334,7 @@ def test_deferred_v_compaction_equals_immediate():
     wl = CONFIGS["llava_ov_7b"].scaled(n_layers=7, budget=784, probe_tokens=64)   # long enough scoring for the move to ride
 
     def run(defer, summary):
-        ls = LockStep(wl, cfg_over=dict(defer_v=defer, summary_token=summary), oracle_over=dict(summary_token=bool(summary)))
+        ls = LockStep(wl, cfg_over=dict(defer_v=defer, defer_k=defer, summary_token=summary), oracle_over=dict(summary_token=bool(summary)))
         ls.fill()
 
         def raw_step(n_probe=None):          # no hermes_get_cache in between (it would flush the pending move)
@@ -289,8 +344,9 @@ def test_deferred_v_compaction_equals_immediate():
         for i in range(5):
             raw_step()                                           # deferred moves ride in the next scoring kernel
             assert hb.hermes_v_pending(ls.h) == defer
+            assert (hb.hermes_k_pending(ls.h) > 0) == bool(defer)
         raw_step(n_probe=2)                                      # G*P = 14 < 32: CUDA-core path -> flush before append
-        assert hb.hermes_v_pending(ls.h) == 0
+        assert hb.hermes_v_pending(ls.h) == 0 and hb.hermes_k_pending(ls.h) == 0
         raw_step()
         torch.cuda.synchronize()
         out = [{k: t.clone() for k, t in hb.hermes_get_cache(ls.h, 0, l).items() if torch.is_tensor(t)}
