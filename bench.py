@@ -141,16 +141,44 @@ def make_pool(wl, rank: int, n_sets: int):
 
 
 # ------------------------------------------------------------------------------- our arm (CUDA)
-def run_ours(args):
+class CudaBackend:
+    """The device plumbing run_ours needs from torch: memory, events, synchronisation, the process group.
+    tests/test_bench_multirank.py substitutes a CPU / gloo stand-in to run the N > 1 path without GPUs."""
+    dist_backend = "nccl"
+
+    def __init__(self, local_rank: int):
+        import torch
+        self.torch = torch
+        torch.cuda.set_device(local_rank)
+        self.dev = torch.device("cuda", local_rank)
+
+    def init_process_group(self, dist):
+        dist.init_process_group(self.dist_backend, device_id=self.dev)
+
+    def event(self):
+        return self.torch.cuda.Event(enable_timing=True)
+
+    def synchronize(self):
+        self.torch.cuda.synchronize()
+
+    def stream_synchronize(self):
+        self.torch.cuda.current_stream().synchronize()
+
+    def pin(self, t):
+        return t.pin_memory()
+
+
+def run_ours(args, backend=None, hb=None):
     import torch
     import torch.distributed as dist
-    import paper_2601_14724_b200 as hb
+    if hb is None:
+        import paper_2601_14724_b200 as hb
 
     rank, local_rank, world = dist_env()
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
+    be = backend if backend is not None else CudaBackend(local_rank)
+    if world > 1 and not dist.is_initialized():
+        be.init_process_group(dist)
+    dev = be.dev
     wl = workload_by_name(args.workload)
     B = wl.n_streams
     tdt = torch.bfloat16 if wl.dtype == "bf16" else torch.float32
@@ -166,7 +194,7 @@ def run_ours(args):
     cfg = hb.config_for_workload(wl, device=local_rank, **over)
     h = hb.hermes_create(cfg)
 
-    host_pool = [tuple(torch.from_numpy(x).to(tdt).pin_memory() for x in s) for s in make_pool(wl, rank, POOL)]
+    host_pool = [tuple(be.pin(torch.from_numpy(x).to(tdt)) for x in s) for s in make_pool(wl, rank, POOL)]
     dev_pool = [tuple(x.to(dev) for x in s) for s in host_pool]
     # fill to the budget without a probe (no eviction), then W warm evicting updates
     n_fill, rem = divmod(wl.budget, wl.chunk_tokens)
@@ -179,13 +207,13 @@ def run_ours(args):
     assert hb.hermes_len(h) == wl.budget
 
     def barrier():
-        torch.cuda.synchronize()
+        be.synchronize()
         if world > 1:
             dist.barrier()
-        torch.cuda.synchronize()
+        be.synchronize()
 
     def timed(n, fn):
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0, e1 = be.event(), be.event()
         barrier()
         e0.record()
         for i in range(n):
@@ -203,7 +231,7 @@ def run_ours(args):
 
     for i in range(max(args.warmup, 3)):
         dev_step(i)
-    sampler = ClockSampler(local_rank) if rank == 0 else None
+    sampler = ClockSampler(local_rank) if rank == 0 and backend is None else None
     ms = timed(args.steps, dev_step)
     clocks = sampler.stop() if sampler else None
     launches = hb.hermes_last_launch_count(h) * args.steps
@@ -220,13 +248,13 @@ def run_ours(args):
     hb.hermes_set_profiling(h, False)
 
     # end to end: HOST (pinned) inputs, H2D + update + D2H of the kept index lists inside the timed region
-    kept_host = torch.zeros(B, wl.n_layers, wl.budget, dtype=torch.int32).pin_memory()
+    kept_host = be.pin(torch.zeros(B, wl.n_layers, wl.budget, dtype=torch.int32))
 
     def host_step(i):
         K, V, Q = host_pool[i % POOL]
         hb.hermes_append_chunk_host(h, K, V, Q, kept_out=kept_host)
         replay.append(i % POOL)
-        torch.cuda.current_stream().synchronize()          # the caller consumes kept_host every step
+        be.stream_synchronize()                              # the caller consumes kept_host every step
 
     n_e2e = min(args.steps, 64)
     for i in range(3):
@@ -250,7 +278,7 @@ def run_ours(args):
         for j in replay:
             K, V, Q = dev_pool[j]
             hb.hermes_append_chunk(h2, K, V, Q)
-        torch.cuda.synchronize()
+        be.synchronize()
         bad = 0
         for b in range(B):
             for l in range(wl.n_layers):
