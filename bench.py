@@ -188,9 +188,7 @@ def run_ours(args, backend=None, hb=None):
     if args.summary_token:
         over.update(summary_token=1)
     if args.no_defer_v:
-        over.update(defer_v=0, defer_k=0)
-    if args.no_defer_k:
-        over.update(defer_k=0)
+        over.update(defer_v=0)
     cfg = hb.config_for_workload(wl, device=local_rank, **over)
     h = hb.hermes_create(cfg)
 
@@ -264,11 +262,11 @@ def run_ours(args, backend=None, hb=None):
     d2h = kept_host.numel() * 4
 
     # outside every timed region: the cache the timed updates left behind must equal, bit for bit, the cache of a
-    # handle that never defers a compaction (defer_v = defer_k = 0; that configuration is the one the lock-step
+    # handle that never defers a compaction (defer_v = 0; that configuration is the one the lock-step
     # oracle tests check) after the same sequence of updates
     check = None
     if not args.no_replay_check:
-        h2 = hb.hermes_create(hb.config_for_workload(wl, device=local_rank, **dict(over, defer_v=0, defer_k=0)))
+        h2 = hb.hermes_create(hb.config_for_workload(wl, device=local_rank, **dict(over, defer_v=0)))
         for i in range(n_fill):
             K, V, _ = dev_pool[i % POOL]
             hb.hermes_append_chunk(h2, K, V, None)
@@ -284,7 +282,7 @@ def run_ours(args, backend=None, hb=None):
             for l in range(wl.n_layers):
                 va, vb = hb.hermes_get_cache(h, b, l), hb.hermes_get_cache(h2, b, l)
                 bad += sum(0 if torch.equal(va[k], vb[k]) else 1 for k in ("k", "v", "pos", "last_kept", "last_scores"))
-        check = {"updates_replayed": len(replay), "against": "defer_v=0, defer_k=0 handle, same inputs",
+        check = {"updates_replayed": len(replay), "against": "defer_v=0 handle, same inputs",
                  "tensors_compared": 5 * B * wl.n_layers, "mismatching_tensors": bad, "bit_identical": bad == 0}
         hb.hermes_destroy(h2)
         if bad:
@@ -320,7 +318,7 @@ def run_ours(args, backend=None, hb=None):
                     exp2={"peak_gexp2_s": xu_peak, "method_gexp2_s": n_exp_method / t_dom / 1e9, "method_frac": n_exp_method / t_dom / 1e9 / xu_peak,
                           "design_gexp2_s": 2 * n_exp_method / t_dom / 1e9, "design_frac": 2 * n_exp_method / t_dom / 1e9 / xu_peak,
                           "note": "XU pipe, 16 exp2/clk/SM x 148 SMs x clocks.max.sm; the design evaluates 2 exp2 per (probe row, token)"},
-                    rides="the previous update's K and V compaction (gather-compaction + rotary correction) is moved inside this launch")
+                    rides="the previous update's V compaction (360 MB) is moved inside this launch")
     elif dom in ("score_stats", "score_colsum"):
         ach = work["flops"] / t_dom / 1e12
         roof = dict(kernel=dom, bound="tensor", achieved=ach, peak=pk["tensor"], unit="TFLOP/s", frac=ach / pk["tensor"], traffic=traffic)
@@ -421,8 +419,7 @@ def main():
     ap.add_argument("--max-position", type=int, default=32768, help="lazy re-indexing: the model's position limit")
     ap.add_argument("--summary-token", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-defer-v", action="store_true", help="compact K and V in the gather kernel instead of inside the next scoring launch")
-    ap.add_argument("--no-defer-k", action="store_true", help="compact K in the gather kernel (V still rides in the next scoring launch)")
+    ap.add_argument("--no-defer-v", action="store_true", help="compact V in the gather kernel instead of inside the next scoring launch")
     ap.add_argument("--no-replay-check", action="store_true", help="skip the post-timing bit-equality check against a non-deferring handle")
     args = ap.parse_args()
     if args.gpus < 1:

@@ -25,6 +25,10 @@
  *     hermes_workspace_bytes() bytes (256-byte aligned), which the handle owns until hermes_destroy().
  *   - Query head h uses KV head h / (n_q_heads / n_kv_heads) (grouped-query attention).
  *   - A handle is not thread-safe; use one per host thread or serialise calls.
+ *   - The tcgen05 scoring kernel is persistent (at most one CTA per SM) and a CTA's second pass waits for row
+ *     statistics written by other CTAs of the same launch, so it needs every CTA of its grid resident at once:
+ *     run it on a device (or an MPS / green-context partition) whose SMs are not shared with other work while an
+ *     update is in flight.
  */
 #ifndef HERMES_H_
 #define HERMES_H_
@@ -93,10 +97,6 @@ typedef struct {
                                    kept V rows to be moved by the NEXT update's scoring kernel (V is not read by
                                    scoring, so the copy hides behind it); hermes_get_cache() and updates that do
                                    not score on tcgen05 first run the pending move on their own.  0: never defer */
-  int32_t defer_k;              /* 1 (default, needs defer_v): the same for K.  The kept K rows of the slabs the next
-                                   scoring launch reaches late are compacted and re-rotated by that launch's mover
-                                   warps (which deliver each slab before its keys are loaded); only the first slabs of
-                                   the schedule are compacted at once.  0: K is always compacted at once            */
   int32_t score_path;           /* HERMES_SCORE_*: AUTO picks tcgen05 when the contraction is dense */
   int32_t device;               /* CUDA device ordinal                                         */
 } hermes_config;
@@ -150,8 +150,8 @@ int hermes_append_chunk_host(hermes_t *h, const void *K_new_host, const void *V_
                              const void *Q_probe_host, int32_t n_new, int32_t n_probe,
                              int32_t pos_start, int32_t *kept_out_host, void *cuda_stream);
 
-/* Fills *out for (stream, layer).  No synchronisation; if a compaction is pending (defer_v / defer_k) it is
- * enqueued on the stream of the last append first.                                                     */
+/* Fills *out for (stream, layer).  No synchronisation; if a V compaction is pending (defer_v) it is enqueued
+ * on the stream of the last append first.                                                              */
 int hermes_get_cache(hermes_t *h, int32_t stream, int32_t layer, hermes_cache_view *out);
 
 /* Host-tracked token count per layer (same for every stream and layer).                              */
@@ -174,9 +174,6 @@ int32_t hermes_last_score_path(const hermes_t *h);
 
 /* 1 if a V compaction is pending (defer_v): the kept V rows of the last eviction have not been moved yet.        */
 int32_t hermes_v_pending(const hermes_t *h);
-
-/* Number of (stream, layer) slabs whose K compaction is pending (defer_k); 0 if none.                             */
-int32_t hermes_k_pending(const hermes_t *h);
 
 /* Number of kernels launched by the last append call.                                                */
 int32_t hermes_last_launch_count(const hermes_t *h);

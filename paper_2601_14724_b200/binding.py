@@ -22,7 +22,7 @@ HERMES_K_NAMES = ("append", "score_stats", "score_combine", "score_colsum", "sel
 
 EXPORTS = ("hermes_default_config", "hermes_workspace_bytes", "hermes_create", "hermes_append_chunk",
            "hermes_append_chunk_host", "hermes_get_cache", "hermes_len", "hermes_device_status",
-           "hermes_set_profiling", "hermes_get_profile", "hermes_last_score_path", "hermes_v_pending", "hermes_k_pending",
+           "hermes_set_profiling", "hermes_get_profile", "hermes_last_score_path", "hermes_v_pending",
            "hermes_last_launch_count", "hermes_destroy", "hermes_last_error")
 
 
@@ -37,7 +37,7 @@ class HermesConfig(C.Structure):
                 ("rope_theta", C.c_float), ("mrope_section", C.c_int32 * 3),
                 ("mrope_compact_axes", C.c_int32), ("mrope_grid_h", C.c_int32),
                 ("mrope_grid_w", C.c_int32), ("pos_offset", C.c_int32), ("reindex_mode", C.c_int32),
-                ("max_position", C.c_int32), ("probe_deep_begin", C.c_int32), ("summary_token", C.c_int32), ("defer_v", C.c_int32), ("defer_k", C.c_int32), ("score_path", C.c_int32),
+                ("max_position", C.c_int32), ("probe_deep_begin", C.c_int32), ("summary_token", C.c_int32), ("defer_v", C.c_int32), ("score_path", C.c_int32),
                 ("device", C.c_int32)]
 
 
@@ -83,7 +83,6 @@ def load_library(rebuild_if_stale: bool = True) -> C.CDLL:
     lib.hermes_last_score_path.argtypes = [vp]
     lib.hermes_last_launch_count.argtypes = [vp]
     lib.hermes_v_pending.argtypes = [vp]
-    lib.hermes_k_pending.argtypes = [vp]
     lib.hermes_destroy.argtypes = [vp]
     lib.hermes_destroy.restype = None
     lib.hermes_last_error.argtypes = [vp]
@@ -249,10 +248,6 @@ def hermes_last_score_path(h: Handle) -> int:
 
 def hermes_v_pending(h: Handle) -> int:
     return int(load_library().hermes_v_pending(h.ptr))
-
-
-def hermes_k_pending(h: Handle) -> int:
-    return int(load_library().hermes_k_pending(h.ptr))
 
 
 def hermes_last_launch_count(h: Handle) -> int:

@@ -48,18 +48,7 @@ struct Geom {
   float* lambda;    // [L] Eq. 7
   int32_t* status;  // sticky device status word
   unsigned* seg_cnt;// [B*L*n_vh_max] tcgen05 scoring: pass-1 progress per group, zeroed by k_append
-  unsigned* kready; // [B*L] rows of a deferred K compaction that have landed in the current buffer, zeroed by k_append
-  int32_t* ord2bl;  // [B*L] processing order of the (stream, layer) slabs -> slab index (see slab_of_order)
 };
-
-// Processing order of the (stream, layer) slabs: the scored ones in the schedule order of the tcgen05 scoring
-// kernel (stream-major, layer ascending), then the shallow ones, which no scoring kernel ever reads.
-__host__ __device__ inline int slab_of_order(const Geom& g, int ord) {
-  const int Ls = g.L - g.n_shallow, ns = g.B * Ls;
-  if (ord < ns) return (ord / Ls) * g.L + g.n_shallow + ord % Ls;
-  const int j = ord - ns;
-  return (j / g.n_shallow) * g.L + j % g.n_shallow;
-}
 
 __host__ __device__ inline size_t slab_index(const Geom& g, int b, int l, int buf) {
   return (size_t(b) * g.L + l) * 2 + buf;

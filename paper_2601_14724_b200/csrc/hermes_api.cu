@@ -16,7 +16,7 @@ static thread_local std::string g_create_error;
 
 namespace {
 template <typename T> struct TypeTag { using type = T; };
-void flush_pending(hermes_t* h, cudaStream_t s);   // runs a deferred K / V compaction on its own
+void flush_v(hermes_t* h, cudaStream_t s);   // runs a deferred V compaction on its own
 }  // namespace
 
 static int fail(hermes_t* h, int code, const char* fmt, ...) {
@@ -51,7 +51,6 @@ extern "C" void hermes_default_config(hermes_config* c) {
   c->score_path = HERMES_SCORE_AUTO;
   c->reindex_mode = HERMES_REINDEX_EAGER;
   c->defer_v = 1;
-  c->defer_k = 1;
 }
 
 extern "C" size_t hermes_workspace_bytes(const hermes_config* c) {
@@ -63,9 +62,6 @@ extern "C" const char* hermes_last_error(const hermes_t* h) { return h ? h->err.
 extern "C" int32_t hermes_len(const hermes_t* h) { return h ? h->len : 0; }
 extern "C" int32_t hermes_last_score_path(const hermes_t* h) { return h ? h->last_score_path : 0; }
 extern "C" int32_t hermes_v_pending(const hermes_t* h) { return h && h->v_pending ? 1 : 0; }
-extern "C" int32_t hermes_k_pending(const hermes_t* h) {
-  return h && h->k_pending ? h->cfg.n_streams * h->cfg.n_layers - h->k_pending_ord0 : 0;
-}
 extern "C" int32_t hermes_last_launch_count(const hermes_t* h) { return h ? h->last_launches : 0; }
 
 extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t bytes, hermes_t** out) {
@@ -137,8 +133,6 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   g.lambda = reinterpret_cast<float*>(h->ws + y.lambda);
   g.status = reinterpret_cast<int32_t*>(h->ws + y.status);
   g.seg_cnt = reinterpret_cast<unsigned*>(h->ws + y.seg_cnt);
-  g.kready = reinterpret_cast<unsigned*>(h->ws + y.kready);
-  g.ord2bl = reinterpret_cast<int32_t*>(h->ws + y.ord2bl);
 
   // per-layer recency weight (Eq. 3-4) and smoothing weight (Eq. 7)
   const int L = c->n_layers, ns = y.n_shallow, nm = y.n_middle;
@@ -167,11 +161,7 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   auto up = [&](void* dst, const void* src, size_t n) { if (e == cudaSuccess) e = cudaMemcpy(dst, src, n, cudaMemcpyHostToDevice); };
   up(g.omega, omega.data(), L * 4); up(g.lambda, lambda.data(), L * 4);
   up(g.rope_freq, freq.data(), half * 8); up(g.rope_tab, tab.data(), tab.size() * 8);
-  {
-    std::vector<int32_t> o2b(size_t(g.B) * L);
-    for (int i = 0; i < g.B * L; ++i) o2b[i] = slab_of_order(g, i);
-    up(g.ord2bl, o2b.data(), o2b.size() * 4);
-  }
+
   if (c->summary_token) {                          // (cos, sin)(delta * theta_j) for every delta Alg. 1 can meet
     std::vector<float2> st(size_t(y.cap + 2) * half);
     for (int r = 0; r < y.cap + 2; ++r)
@@ -183,7 +173,6 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   }
   if (e == cudaSuccess) e = cudaMemset(g.status, 0, 256);
   if (e == cudaSuccess) e = cudaMemset(h->ws + y.seg_cnt, 0, size_t(g.B) * L * y.n_vh_max * 4);
-  if (e == cudaSuccess) e = cudaMemset(g.kready, 0, size_t(g.B) * L * 4);
   if (e == cudaSuccess) e = cudaMemset(g.posc, 0, size_t(g.B) * L * 2 * y.n_axes * y.cap * 4);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_select, cudaFuncAttributeMaxDynamicSharedMemorySize, y.cap * 4);
   if (e == cudaSuccess) e = cudaDeviceSynchronize();
@@ -249,10 +238,10 @@ extern "C" int hermes_get_cache(hermes_t* h, int32_t stream, int32_t layer, herm
   if (stream < 0 || stream >= h->cfg.n_streams || layer < 0 || layer >= h->cfg.n_layers)
     return fail(h, HERMES_EINVAL, "stream %d / layer %d out of range", stream, layer);
   const Geom& g = h->geom;
-  if (h->v_pending || h->k_pending) {       // make the cache whole before handing out pointers (stream of the last append)
-    flush_pending(h, static_cast<cudaStream_t>(h->last_stream));
+  if (h->v_pending) {                       // make V whole before handing out pointers (stream of the last append)
+    flush_v(h, static_cast<cudaStream_t>(h->last_stream));
     const cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return fail(h, HERMES_ECUDA, "deferred compaction: %s", cudaGetErrorString(e));
+    if (e != cudaSuccess) return fail(h, HERMES_ECUDA, "V compaction: %s", cudaGetErrorString(e));
   }
   const size_t bl = size_t(stream) * g.L + layer, slab = bl * 2 + h->cur;
   out->k = static_cast<char*>(g.kc) + slab * g.cap * h->lay.row_bytes;
@@ -295,13 +284,11 @@ void launch_simt(hermes_t* h, const void* q, int Tn, int P, float scale_log2, cu
   else if (g.d == 64) run(std::integral_constant<int, 64>{});
   else run(std::integral_constant<int, 128>{});
 }
-// k_gather for buffer `buf` -> buf ^ 1 in the given mode (kGatherKV / kGatherK / kGatherV), slabs [ord0, ord1) of the
-// processing order (slab_of_order).
-void launch_gather(hermes_t* h, int mode, int buf, cudaStream_t s, int ord0, int ord1) {
+// k_gather for buffer `buf` -> buf ^ 1 in the given mode (kGatherKV / kGatherK / kGatherV).
+void launch_gather(hermes_t* h, int mode, int buf, cudaStream_t s) {
   const hermes_config& c = h->cfg;
   const Geom& g = h->geom;
-  const int BL = ord1 - ord0;
-  if (BL <= 0) return;
+  const int BL = g.B * g.L;
   ++h->last_launches;
   const int V = c.dtype == HERMES_BF16 ? 8 : 4;
   const int upr = g.Hkv * (g.d / 2 / V);
@@ -314,7 +301,7 @@ void launch_gather(hermes_t* h, int mode, int buf, cudaStream_t s, int ord0, int
   const dim3 grid(gx, BL), block(kGatherThreads);
   auto go = [&](auto tag, auto nax, auto md) {
     using T = typename decltype(tag)::type;
-    launch_pdl(k_gather<T, decltype(nax)::value, decltype(md)::value>, grid, block, 0, s, g, buf, ord0);
+    launch_pdl(k_gather<T, decltype(nax)::value, decltype(md)::value>, grid, block, 0, s, g, buf);
   };
   auto by_mode = [&](auto tag, auto nax) {
     if (mode == kGatherKV) go(tag, nax, std::integral_constant<int, kGatherKV>{});
@@ -329,12 +316,11 @@ void launch_gather(hermes_t* h, int mode, int buf, cudaStream_t s, int ord0, int
   else by_axes(TypeTag<float>{});
 }
 
-// Runs a deferred K / V compaction on its own (no scoring kernel to carry it).
-void flush_pending(hermes_t* h, cudaStream_t s) {
-  const int n_ord = h->geom.B * h->geom.L;
-  if (h->k_pending) launch_gather(h, kGatherK, h->pend_src_buf, s, h->k_pending_ord0, n_ord);
-  if (h->v_pending) launch_gather(h, kGatherV, h->pend_src_buf, s, 0, n_ord);
-  h->k_pending = h->v_pending = false;
+// Runs a deferred V compaction on its own (no scoring kernel to carry it).
+void flush_v(hermes_t* h, cudaStream_t s) {
+  if (!h->v_pending) return;
+  launch_gather(h, kGatherV, h->v_src_buf, s);
+  h->v_pending = false;
 }
 }  // namespace
 
@@ -384,10 +370,10 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
   const bool use_tc = evict && g.L > g.n_shallow && h->tc_ok && c.score_path != HERMES_SCORE_SIMT &&
                       (c.score_path == HERMES_SCORE_TCGEN05 || tc_profitable(h, Tn, n_probe));
   h->last_stream = cuda_stream;
-  // a pending compaction rides in this update's scoring kernel if that kernel is long enough and has the
+  // a pending V compaction rides in this update's scoring kernel if that kernel is long enough and has the
   // shared memory for it; otherwise it runs on its own first
-  const bool ride = use_tc && tc_ride_ok(h, Tn, n_probe);
-  if (!ride) flush_pending(h, s);
+  const bool ride = use_tc && tc_v_ride_ok(h, Tn, n_probe);
+  if (!ride) flush_v(h, s);
   {
     Prof p(h, HERMES_K_APPEND, s);
     const size_t n_vec = size_t(n_new) * row_vecs;
@@ -410,8 +396,8 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
     const float scale_log2 = scale * kLog2e;
     if (g.L > g.n_shallow) {
       if (use_tc) {
-        if (int rc = tc_score(h, Q_probe, Tn, n_probe, scale_log2, s, ride && h->v_pending, ride && h->k_pending)) return rc;
-        h->v_pending = h->k_pending = false;
+        if (int rc = tc_score(h, Q_probe, Tn, n_probe, scale_log2, s, ride && h->v_pending)) return rc;
+        h->v_pending = false;
         h->last_score_path = HERMES_SCORE_TCGEN05;
       } else {
         if (c.dtype == HERMES_BF16) launch_simt<__nv_bfloat16>(h, Q_probe, Tn, n_probe, scale_log2, s);
@@ -440,16 +426,10 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
     }
     {
       if (h->profiling) { cudaEventRecord(h->timer.beg[HERMES_K_GATHER], s); h->timer.ran[HERMES_K_GATHER] = true; }
-      // on the tcgen05 path V stays behind, and so does K of every slab but the first k_now of the processing order: the
-      // next update's scoring kernel compacts them (tc_mover), or a flush
+      // on the tcgen05 path V stays behind: the next update's scoring kernel compacts it (tc_v_mover), or a flush
       const bool defer_v = ride && c.defer_v != 0;   // the next update will most likely look like this one
-      const int n_ord = g.B * g.L;
-      const int k_now = defer_v ? tc_k_now(h, Tn, n_probe) : n_ord;
-      launch_gather(h, defer_v ? kGatherK : kGatherKV, h->cur, s, 0, k_now);
-      if (defer_v) {
-        h->v_pending = true; h->pend_src_buf = h->cur;
-        h->k_pending = k_now < n_ord; h->k_pending_ord0 = k_now;
-      }
+      launch_gather(h, defer_v ? kGatherK : kGatherKV, h->cur, s);
+      if (defer_v) { h->v_pending = true; h->v_src_buf = h->cur; }
       if (h->profiling) cudaEventRecord(h->timer.end[HERMES_K_GATHER], s);
     }
   }

@@ -17,7 +17,7 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {           // byte offsets into the workspace
   size_t kc, vc, posc, colsum, wsum, wmax, rowstat, partial, scores, kept, delta, evicted, rope_tab, rope_freq, sum_tab, omega, lambda,
-      status, seg_cnt, kready, ord2bl, stage_k, stage_v, stage_q, tmaps, total;
+      status, seg_cnt, stage_k, stage_v, stage_q, tmaps, total;
   int cap, n_axes, n_part_max, table_rows, n_shallow, n_middle, n_deep, n_vh_max;
   size_t esize, row_bytes;
 };
@@ -60,8 +60,6 @@ inline const char* validate(const hermes_config& c) {
   if (c.reindex_mode != HERMES_REINDEX_EAGER && c.reindex_mode != HERMES_REINDEX_LAZY) return "bad reindex_mode";
   if (c.probe_deep_begin < 0 || c.probe_deep_begin >= c.max_probe_tokens) return "probe_deep_begin must lie in [0, max_probe_tokens)";
   if (c.defer_v != 0 && c.defer_v != 1) return "defer_v must be 0 or 1";
-  if (c.defer_k != 0 && c.defer_k != 1) return "defer_k must be 0 or 1";
-  if (c.defer_k && !c.defer_v) return "defer_k needs defer_v";
   if (c.summary_token != 0 && c.summary_token != 1) return "summary_token must be 0 or 1";
   if (c.summary_token && (c.rope_mode != HERMES_ROPE_1D || c.reindex_mode != HERMES_REINDEX_EAGER || c.budget < 2))
     return "summary tokens need 1D RoPE, eager re-indexing and budget >= 2";
@@ -119,8 +117,6 @@ inline Layout make_layout(const hermes_config& c) {
   y.lambda = take(size_t(c.n_layers) * 4);
   y.status = take(256);
   y.seg_cnt = take(BL * y.n_vh_max * 4);
-  y.kready = take(BL * 4);
-  y.ord2bl = take(BL * 4);
   y.stage_k = take(BL * c.max_chunk_tokens * y.row_bytes);
   y.stage_v = take(BL * c.max_chunk_tokens * y.row_bytes);
   y.stage_q = take(BL * rows * c.head_dim * y.esize);
@@ -165,13 +161,10 @@ struct hermes {
   cudaStream_t side_stream = nullptr;   // host entry point: V's host-to-device copy (created on first use)
   cudaEvent_t ev_k_done = nullptr, ev_v_done = nullptr;
   int n_vh = 0;             // column-sum slots written by the last scoring pass
-  // deferred compaction: after an eviction on the tcgen05 path k_gather moves only the K rows of the first
-  // k_pending_ord0 slabs (processing order, slab_of_order); the other kept K rows and all kept V rows still sit in
-  // buffer pend_src_buf and are moved into the current buffer by the NEXT update's scoring kernel (or by a flush)
+  // deferred V compaction: after an eviction on the tcgen05 path k_gather moves only K; the kept V rows still sit
+  // in buffer v_src_buf and are moved into the current buffer by the NEXT update's scoring kernel (or by a flush)
   bool v_pending = false;
-  bool k_pending = false;
-  int k_pending_ord0 = 0;
-  int pend_src_buf = 0;
+  int v_src_buf = 0;
   void* last_stream = nullptr;
   bool profiling = false;
   bool tc_ok = false;       // tcgen05 scoring path usable for this config + device

@@ -16,8 +16,8 @@ k_append(Geom g, const uint4* __restrict__ k_new, const uint4* __restrict__ v_ne
   pdl_launch_dependents();
   const int bl = blockIdx.y;                        // b * L + l
   const bool do_k = what & kAppendK, do_v = what & kAppendV;
-  if (do_k && blockIdx.x == 0) {                     // per-update counters of this slab: max of W, pass-1 progress, K rows delivered
-    if (threadIdx.x == 0) { g.wmax[bl] = 0u; g.kready[bl] = 0u; }
+  if (do_k && blockIdx.x == 0) {                     // per-update counters of this slab: max of W, pass-1 progress of the tcgen05 scoring
+    if (threadIdx.x == 0) g.wmax[bl] = 0u;
     for (int i = threadIdx.x; i < g.n_vh_max; i += blockDim.x) g.seg_cnt[size_t(bl) * g.n_vh_max + i] = 0u;
   }
   const size_t slab = size_t(bl) * 2 + cur;

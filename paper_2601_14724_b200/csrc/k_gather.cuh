@@ -72,19 +72,18 @@ __device__ __forceinline__ void rotate_unit(const Geom& g, const int (&dl)[NAX],
   hi = Elem<T>::pack(y);
 }
 
-// grid = (blocks per slab, slabs); block row y handles the slab of processing order ord0 + y (slab_of_order); each
-// thread walks units idx, idx + stride, ... of its (stream, layer).
+// grid = (blocks per slab, B*L); each thread walks units idx, idx + stride, ... of its (stream, layer).
 // kMode: kGatherKV moves K and V; kGatherK only K (V's compaction is deferred into the next update's scoring
 // kernel, see tc_v_mover in k_score_tc.cuh); kGatherV only V (flush of a deferred compaction).
 constexpr int kGatherKV = 0, kGatherK = 1, kGatherV = 2;
 
 template <typename T, int NAX, int kMode>
 __global__ void __launch_bounds__(kGatherThreads, 4)
-k_gather(Geom g, int cur, int ord0) {
+k_gather(Geom g, int cur) {
   pdl_wait();
   pdl_launch_dependents();
   constexpr int V = Elem<T>::kPerVec;
-  const int bl = __ldg(g.ord2bl + ord0 + blockIdx.y);
+  const int bl = blockIdx.y;
   const int half = g.d >> 1;
   const int uph = half / V;                                 // units per head
   const int upr = g.Hkv * uph;                              // units per token row

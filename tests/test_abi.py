@@ -24,8 +24,8 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_config_struct_matches_header_size():
-    # 15 int32 + 3 float + int32 + 4 float + int32 + float + 3 int32 + 12 int32 = 40 x 4 bytes
-    assert C.sizeof(hb.HermesConfig) == 40 * 4
+    # 15 int32 + 3 float + int32 + 4 float + int32 + float + 3 int32 + 11 int32 = 39 x 4 bytes
+    assert C.sizeof(hb.HermesConfig) == 39 * 4
     assert hb.hermes_default_config().reindex_mode == 0
     cfg = hb.hermes_default_config()
     assert (cfg.omega0, cfg.gamma) == (0.75, pytest.approx(0.6))
