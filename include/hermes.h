@@ -90,9 +90,10 @@ typedef struct {
                                    [local prompt | global prompt], middle layers use all (App. B);
                                    0 = all rows everywhere                                              */
   int32_t summary_token;        /* 1: every deep layer keeps budget-1 tokens by Top-K and appends ONE summary
-                                   token of the evicted ones (Alg. 1) in slot budget-1 at
-                                   position pos_offset+budget-1; last_kept[budget-1] = -1 marks it.  Needs
-                                   HERMES_ROPE_1D and HERMES_REINDEX_EAGER                              */
+                                   token of the evicted ones (Alg. 1) in slot budget-1;
+                                   last_kept[budget-1] = -1 marks it.  Its position: pos_offset+budget-1 at a step that
+                                   re-indexes; under LAZY re-indexing, between re-index steps, the position after the
+                                   newest token (the next chunk then starts one position later).  Needs HERMES_ROPE_1D  */
   int32_t defer_v;              /* 1 (default): on the tcgen05 path an eviction compacts K at once but leaves the
                                    kept V rows to be moved by the NEXT update's scoring kernel (V is not read by
                                    scoring, so the copy hides behind it); hermes_get_cache() and updates that do

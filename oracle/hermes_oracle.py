@@ -432,20 +432,25 @@ def oracle_step(st: OracleStream, K_new: np.ndarray, V_new: np.ndarray,
     pos_new = np.zeros((L, cfg.n_axes, cfg.budget), np.int64)
     K_out = np.zeros((L, cfg.budget) + st.K.shape[2:], np.float32)
     V_out = np.zeros_like(K_out)
-    reindex = cfg.reindex_mode == "eager" or lazy_reindex_due(cfg, p_end)
-    if cfg.summary_token and (cfg.rope_mode != "1d" or cfg.reindex_mode != "eager"):
-        raise ValueError("summary tokens are defined here for eager 1D re-indexing only (DESIGN f1)")
+    if cfg.summary_token and cfg.rope_mode != "1d":
+        raise ValueError("summary tokens are defined here for 1D RoPE only: Alg. 1 takes ONE target index t (DESIGN f1)")
+    # a summary token takes a position of its own: under lazy re-indexing the position after the newest token
+    # (DESIGN f1/f2), so the running position counter -- and with it the re-index trigger -- advances by one more
+    summ_pos = 1 if (cfg.summary_token and stage_split(cfg.n_layers, cfg.n_shallow, cfg.n_deep)[2] > 0) else 0
+    reindex = cfg.reindex_mode == "eager" or lazy_reindex_due(cfg, p_end + summ_pos)
     for l in range(L):
         if cfg.summary_token and layer_stage(cfg, l) == "deep":
             # deep layers keep |M| - 1 tokens by Top-K and append ONE summary token of everything evicted, so the
             # layer still holds exactly |M| tokens; it sits after the kept tokens
-            # (Alg. 1 step 3) at the next contiguous position t = offset + |M| - 1 and is an ordinary,
-            # evictable token from then on (DESIGN f1).  kept[l][-1] = -1 marks it.
+            # (Alg. 1 step 3) and is an ordinary, evictable token from then on (DESIGN f1).  kept[l][-1] = -1 marks
+            # it.  Its position t: at a re-index step the next contiguous one, offset + |M| - 1; between re-index
+            # steps of the lazy mode the kept tokens keep their original indices and t is the position after the
+            # newest token, p_end (PAPER.md:126-128 with Alg. 1 step 3: positions stay strictly increasing).
             I = select_topk(S_tilde[l], cfg.budget - 1)
             ev = np.setdiff1d(np.arange(T), I)
             p_old = st.pos[l][:, I]
-            p_new = compact_positions(cfg, p_old)
-            t = cfg.pos_offset + cfg.budget - 1
+            p_new = compact_positions(cfg, p_old) if reindex else p_old
+            t = cfg.pos_offset + cfg.budget - 1 if reindex else p_end
             k_sum, v_sum = summary_token(cfg, st.K[l, ev], st.V[l, ev], st.pos[l][:, ev], t)
             kept[l, :-1], kept[l, -1] = I, -1
             pos_new[l][:, :-1], pos_new[l][:, -1] = p_new, t
@@ -464,6 +469,8 @@ def oracle_step(st: OracleStream, K_new: np.ndarray, V_new: np.ndarray,
     st.len = cfg.budget                                        # 9.
     if reindex:                       # every position is now below offset + |M| (M-RoPE: + min(steps seen, |M|))
         st.next_pos = cfg.pos_offset + (cfg.budget if cfg.rope_mode == "1d" else min(st.t_steps_seen, cfg.budget))
+    else:
+        st.next_pos = p_end + summ_pos
     st.last = {"T": T, "evicted": True, "reindexed": reindex, "W": W, "S": S, "S_tilde": S_tilde,
                "kept": kept, "pos_new": pos_new}
     return st.last

@@ -42,8 +42,9 @@ struct Geom {
   int32_t* evicted; // [B*L][n_evict_max] ascending evicted indices (summary-token layers only)
   float2* rope_tab; // [table_rows][d/2] (cos, sin)(-r * theta_j) for r = row index
   double* rope_freq;// [d/2] theta_j in fp64 (slow path for deltas outside the table)
-  float2* sum_tab;  // summary tokens: [cap + 2][d/2] (cos, sin)(delta * theta_j), delta = row - sum_tab_zero
+  float2* sum_tab;  // summary tokens: [sum_tab_rows][d/2] (cos, sin)(delta * theta_j), delta = row - sum_tab_zero
   int sum_tab_zero; // row of delta = 0 in sum_tab
+  int sum_tab_rows;
   float* omega;     // [L] weight of the recency term (Eq. 3-4); 1 shallow, 0 deep
   float* lambda;    // [L] Eq. 7
   int32_t* status;  // sticky device status word

@@ -128,7 +128,7 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   g.rope_tab = reinterpret_cast<float2*>(h->ws + y.rope_tab);
   g.rope_freq = reinterpret_cast<double*>(h->ws + y.rope_freq);
   g.sum_tab = reinterpret_cast<float2*>(h->ws + y.sum_tab);
-  g.sum_tab_zero = y.cap - c->budget + 1;        // deltas of the summary alignment lie in [-(cap - budget + 1), budget)
+  g.sum_tab_zero = y.sum_tab_neg; g.sum_tab_rows = y.sum_tab_rows;
   g.omega = reinterpret_cast<float*>(h->ws + y.omega);
   g.lambda = reinterpret_cast<float*>(h->ws + y.lambda);
   g.status = reinterpret_cast<int32_t*>(h->ws + y.status);
@@ -163,8 +163,8 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   up(g.rope_freq, freq.data(), half * 8); up(g.rope_tab, tab.data(), tab.size() * 8);
 
   if (c->summary_token) {                          // (cos, sin)(delta * theta_j) for every delta Alg. 1 can meet
-    std::vector<float2> st(size_t(y.cap + 2) * half);
-    for (int r = 0; r < y.cap + 2; ++r)
+    std::vector<float2> st(size_t(y.sum_tab_rows) * half);
+    for (int r = 0; r < y.sum_tab_rows; ++r)
       for (int j = 0; j < half; ++j) {
         const double ang = double(r - g.sum_tab_zero) * freq[j];
         st[size_t(r) * half + j] = make_float2(float(std::cos(ang)), float(std::sin(ang)));
@@ -359,7 +359,9 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
   // lazy mode: re-index only when the next chunk would no longer fit below max_position
   const long long span_max = g.n_axes == 1 ? c.max_chunk_tokens
                                            : (c.max_chunk_tokens + c.mrope_grid_h * c.mrope_grid_w - 1) / (c.mrope_grid_h * c.mrope_grid_w);
-  const bool reindex = !lazy || p0 + span + span_max > c.max_position;
+  // a summary token takes the position after the newest token (DESIGN f1): the running counter advances by one more
+  const int summ_pos = (c.summary_token && h->lay.n_deep > 0) ? 1 : 0;
+  const bool reindex = !lazy || p0 + span + summ_pos + span_max > c.max_position;
   if (lazy && p0 + span > c.max_position) return fail(h, HERMES_ECAPACITY, "positions would exceed max_position %d", c.max_position);
 
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
@@ -414,14 +416,16 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
       const float r_norm_sum = float((1.0 - std::exp(-k)) / (1.0 - std::exp(-k * Tn)));
       if (g.L > g.n_shallow)
         launch_pdl(k_wsum, dim3((Tn + 255) / 256, g.B * (g.L - g.n_shallow)), dim3(256), 0, s, g, Tn, n_probe, h->n_vh);
-      launch_pdl(k_select, dim3(BL), dim3(kSelThreads), size_t(Tn) * 4, s, g, h->cur, Tn, c.forget_rate, int(c.norm_mode == HERMES_NORM_SUM), r_norm_sum, int(reindex));
+      launch_pdl(k_select, dim3(BL), dim3(kSelThreads), size_t(Tn) * 4, s, g, h->cur, Tn, c.forget_rate, int(c.norm_mode == HERMES_NORM_SUM), r_norm_sum, int(reindex),
+                 reindex ? c.pos_offset + c.budget - 1 : int(p0 + span));
     }
     if (c.summary_token && h->lay.n_deep > 0) {
       Prof p(h, HERMES_K_SUMMARY, s);
       const dim3 sgrid(g.Hkv, g.B * h->lay.n_deep), sblock(64 * kSumLanes);
       const size_t ssm = size_t(Tn - c.budget + 1) * 8;
-      const cudaError_t es = c.dtype == HERMES_BF16 ? launch_pdl(k_summary<__nv_bfloat16>, sgrid, sblock, ssm, s, g, h->cur, Tn)
-                                                    : launch_pdl(k_summary<float>, sgrid, sblock, ssm, s, g, h->cur, Tn);
+      const int st_pos = reindex ? c.pos_offset + c.budget - 1 : int(p0 + span);
+      const cudaError_t es = c.dtype == HERMES_BF16 ? launch_pdl(k_summary<__nv_bfloat16>, sgrid, sblock, ssm, s, g, h->cur, Tn, st_pos)
+                                                    : launch_pdl(k_summary<float>, sgrid, sblock, ssm, s, g, h->cur, Tn, st_pos);
       if (es != cudaSuccess) return fail(h, HERMES_ECUDA, "summary kernel launch: %s", cudaGetErrorString(es));
     }
     {
@@ -439,7 +443,7 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
   if (g.n_axes == 3) h->t_steps_seen += steps;
   if (evict) {
     h->cur ^= 1; h->len = c.budget; h->last_T = Tn;
-    if (!reindex) h->next_pos = p0 + span; else
+    if (!reindex) h->next_pos = p0 + span + summ_pos; else
     // after eager re-indexing every cached position is below offset + budget (1D) or below
     // offset + min(temporal steps seen, budget) (M-RoPE: a layer holds at most that many distinct t)
     h->next_pos = c.pos_offset + (g.n_axes == 1 ? (long long)c.budget : std::min<long long>(h->t_steps_seen, c.budget));

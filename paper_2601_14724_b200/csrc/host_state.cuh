@@ -18,7 +18,7 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 struct Layout {           // byte offsets into the workspace
   size_t kc, vc, posc, colsum, wsum, wmax, rowstat, partial, scores, kept, delta, evicted, rope_tab, rope_freq, sum_tab, omega, lambda,
       status, seg_cnt, stage_k, stage_v, stage_q, tmaps, total;
-  int cap, n_axes, n_part_max, table_rows, n_shallow, n_middle, n_deep, n_vh_max;
+  int cap, n_axes, n_part_max, table_rows, n_shallow, n_middle, n_deep, n_vh_max, sum_tab_neg, sum_tab_rows;
   size_t esize, row_bytes;
 };
 
@@ -61,8 +61,8 @@ inline const char* validate(const hermes_config& c) {
   if (c.probe_deep_begin < 0 || c.probe_deep_begin >= c.max_probe_tokens) return "probe_deep_begin must lie in [0, max_probe_tokens)";
   if (c.defer_v != 0 && c.defer_v != 1) return "defer_v must be 0 or 1";
   if (c.summary_token != 0 && c.summary_token != 1) return "summary_token must be 0 or 1";
-  if (c.summary_token && (c.rope_mode != HERMES_ROPE_1D || c.reindex_mode != HERMES_REINDEX_EAGER || c.budget < 2))
-    return "summary tokens need 1D RoPE, eager re-indexing and budget >= 2";
+  if (c.summary_token && (c.rope_mode != HERMES_ROPE_1D || c.budget < 2))
+    return "summary tokens need 1D RoPE (Alg. 1 takes one target index t) and budget >= 2";
   if (c.reindex_mode == HERMES_REINDEX_LAZY) {
     const long long span = c.rope_mode == HERMES_ROPE_M3D
         ? (c.max_chunk_tokens + c.mrope_grid_h * c.mrope_grid_w - 1) / (c.mrope_grid_h * c.mrope_grid_w) : c.max_chunk_tokens;
@@ -112,7 +112,17 @@ inline Layout make_layout(const hermes_config& c) {
   y.evicted = take(BL * size_t(y.cap - c.budget + 1) * 4);
   y.rope_tab = take(size_t(y.table_rows) * (c.head_dim / 2) * 8);
   y.rope_freq = take(size_t(c.head_dim / 2) * 8);
-  y.sum_tab = take(c.summary_token ? size_t(y.cap + 2) * (c.head_dim / 2) * 8 : 0);
+  // summary tokens: (cos, sin)(delta * theta_j) for delta in [-sum_tab_neg, sum_tab_rows - sum_tab_neg).  Eager: an evicted
+  // token moves from p in [offset, offset + cap) to t = offset + budget - 1.  Lazy: to the position after the newest token
+  // (delta up to max_position - offset), and back down at a re-index step.  Capped at 2 x 65536 rows; beyond: fp64 sincos.
+  y.sum_tab_neg = y.cap - c.budget + 1;
+  int sum_pos = c.budget + 1;
+  if (c.reindex_mode == HERMES_REINDEX_LAZY) {
+    y.sum_tab_neg = std::min(65536, std::max(y.sum_tab_neg, c.max_position - c.pos_offset + 1));
+    sum_pos = std::min(65536, std::max(sum_pos, c.max_position - c.pos_offset + 1));
+  }
+  y.sum_tab_rows = c.summary_token ? y.sum_tab_neg + sum_pos : 0;
+  y.sum_tab = take(size_t(y.sum_tab_rows) * (c.head_dim / 2) * 8);
   y.omega = take(size_t(c.n_layers) * 4);
   y.lambda = take(size_t(c.n_layers) * 4);
   y.status = take(256);

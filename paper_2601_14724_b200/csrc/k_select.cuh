@@ -109,7 +109,7 @@ k_wsum(Geom g, int Tn, int P, int n_vh) {
 }
 
 __global__ void __launch_bounds__(kSelThreads)
-k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum, int reindex) {
+k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum, int reindex, int summary_pos) {
   extern __shared__ float s_sc[];                    // [Tn] smoothed scores
   // per-warp digit histograms (radix phase); the M-RoPE rank bitmap + word prefixes reuse the space later
   __shared__ __align__(16) int whist[32 * 256];
@@ -311,7 +311,7 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
   if (blockIdx.x == 5 && threadIdx.x == 0) printf("select phases (cycles): setup %lld scores %lld radix %lld count+scan %lld write %lld\n", tstamp[1]-tstamp[0], tstamp[2]-tstamp[1], tstamp[3]-tstamp[2], tstamp[6]-tstamp[4], tstamp[5]-tstamp[6]);
 #endif
   if (summ && tid == 0) {                               // the summary token's slot (filled by k_summary)
-    kept[n_keep] = -1; pos_new[n_keep] = g.pos_offset + n_keep; dl1[n_keep] = 0;
+    kept[n_keep] = -1; pos_new[n_keep] = summary_pos; dl1[n_keep] = 0;
   }
   if (g.n_axes == 1) return;
   __syncthreads();                                      // kept[] visible to the whole block

@@ -1,9 +1,10 @@
 // f1 -- summary token of the evicted tokens of every deep layer (Alg. 1):
-//   v_sum = Mean(V_p);  k_sum = Mean(ApplyDelta(K_p, RotaryDelta(P_p -> t))),  t = pos_offset + budget - 1,
+//   v_sum = Mean(V_p);  k_sum = Mean(ApplyDelta(K_p, RotaryDelta(P_p -> t))),  t = pos_offset + budget - 1 at a re-index
+//   step, the position after the newest token between the re-index steps of the lazy mode (DESIGN f1),
 // written to slot budget-1 of the NEW buffer (k_gather leaves that slot alone; k_select set its position).
 // One block per (KV head, stream x deep layer): thread = (rotary pair j, token lane q); token lane q walks the
 // evicted tokens q, q + kSumLanes, ...  (cos, sin) from a table built in fp64 at create time for every delta in
-// [-(cap - budget + 1), budget) (fp64 sincos otherwise), rotation in fp32 without FMA exactly as in k_gather, sums in fp64, lanes reduced
+// the table range (fp64 sincos otherwise), rotation in fp32 without FMA exactly as in k_gather, sums in fp64, lanes reduced
 // in shared memory in fixed order, one rounding to the storage dtype.  ~E x 2 KB per layer: latency only.
 #pragma once
 #include "common.cuh"
@@ -14,7 +15,7 @@ constexpr int kSumLanes = 16;
 
 template <typename T>
 __global__ void __launch_bounds__(64 * kSumLanes)
-k_summary(Geom g, int cur, int Tn) {
+k_summary(Geom g, int cur, int Tn, int t) {
   __shared__ double red[kSumLanes][4][64];                 // [token lane][kx, ky, vx, vy][pair]
   extern __shared__ int s_list[];                          // [2][n_ev]: source row, rotary delta of every evicted token
   pdl_wait();
@@ -25,7 +26,6 @@ k_summary(Geom g, int cur, int Tn) {
   const int b = blockIdx.y / g.n_deep, l = g.L - g.n_deep + blockIdx.y % g.n_deep;
   const int bl = b * g.L + l;
   const int n_keep = g.budget - 1, n_ev = Tn - n_keep;
-  const int t = g.pos_offset + n_keep;
   const size_t slab_src = size_t(bl) * 2 + cur, slab_dst = size_t(bl) * 2 + (cur ^ 1);
   const T* ks = reinterpret_cast<const T*>(g.kc) + slab_src * g.cap * g.row_elems + kvh * g.d;
   const T* vs = reinterpret_cast<const T*>(g.vc) + slab_src * g.cap * g.row_elems + kvh * g.d;
@@ -48,7 +48,7 @@ k_summary(Geom g, int cur, int Tn) {
         const int delta = s_dl[i];
         const int r = delta + g.sum_tab_zero;
         float c, s;
-        if (r >= 0 && r < g.cap + 2) { const float2 cs = __ldg(g.sum_tab + size_t(r) * half + jj); c = cs.x; s = cs.y; }
+        if (r >= 0 && r < g.sum_tab_rows) { const float2 cs = __ldg(g.sum_tab + size_t(r) * half + jj); c = cs.x; s = cs.y; }
         else { const double ang = double(delta) * g.rope_freq[jj]; c = float(cos(ang)); s = float(sin(ang)); }   // explicit pos_start jumps
         const size_t o = size_t(src) * g.row_elems;
         const float x = Elem<T>::to_float(__ldcg(ks + o + jj)), y = Elem<T>::to_float(__ldcg(ks + o + jj + half));

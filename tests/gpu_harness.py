@@ -86,8 +86,9 @@ class LockStep:
             span = (n_new + tpt - 1) // tpt
             self.t_steps_seen += span
         c = self.ocfg
-        self.next_pos = p0 + span
-        if evicted and (c.reindex_mode == "eager" or ho.lazy_reindex_due(c, p0 + span)):
+        summ = 1 if (evicted and c.summary_token and ho.stage_split(c.n_layers, c.n_shallow, c.n_deep)[2] > 0) else 0
+        self.next_pos = p0 + span + summ
+        if evicted and (c.reindex_mode == "eager" or ho.lazy_reindex_due(c, p0 + span + summ)):
             self.next_pos = c.pos_offset + (c.budget if c.rope_mode == "1d" else min(self.t_steps_seen, c.budget))
         if not track_ids:
             return

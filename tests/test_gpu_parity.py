@@ -149,6 +149,26 @@ def test_sweep_corners_reduced_layers():
         ls.close()
 
 
+def test_sweep_32k_budget_point_full_layers():
+    """configs[3], the largest budget (32 768 tokens per layer, T = 32 964) at all 28 layers with 64 probe rows:
+    k_select with 129 KB of dynamic shared memory and 2 flag chunks per thread, 258 token tiles per group."""
+    wl = sweep_point(32768, 64)
+    ls, reps = _run(wl, 1)
+    assert reps[0]["T"] == 32768 + 196 and hb.hermes_last_score_path(ls.h) == hb.HERMES_SCORE_TCGEN05
+    ls.close()
+
+
+def test_batched_72b_full_size_schedule():
+    """configs[4] at full size (80 layers x 16 streams, 64 q / 8 kv heads, budget 4096): SURVEY.md 8(d)'s parity
+    schedule -- streams {0, 7, 15} compared with the oracle on 2 evicting updates (the second one with the first
+    one's V compaction pending until the lock-step download flushes it)."""
+    wl = CONFIGS["batched_72b"]
+    ls, reps = _run(wl, 2, streams=[0, 7, 15])
+    assert len(reps) == 6 and all(r["T"] == 4096 + 196 for r in reps)
+    assert hb.hermes_last_score_path(ls.h) == hb.HERMES_SCORE_TCGEN05
+    ls.close()
+
+
 def test_batched_72b_geometry_reduced_equals_single_streams():
     """configs[4] geometry (64 q / 8 kv heads), 3 streams x 8 layers: oracle parity per stream, and the
     batched call equals B single-stream calls bit for bit."""
@@ -315,6 +335,23 @@ def test_summary_token_toy_and_bf16():
     ls, reps = _run(wl, 3, n_warm=1, cfg_over=dict(summary_token=1), oracle_over=dict(summary_token=True))
     assert all(r.get("summary_layers") == 2 for r in reps)
     ls.close()
+
+
+def test_summary_token_under_lazy_reindexing():
+    """The paper's streaming configuration of the management path: lazy re-indexing with the
+    deep-layer summary token at every compression step.  Kept keys are copied, the summary token is
+    aligned to the position after the newest token; the re-index step in the middle re-rotates everything."""
+    wl = CONFIGS["toy"]
+    ls, reps = _run(wl, 8, cfg_over=dict(summary_token=1, reindex_mode=hb.HERMES_REINDEX_LAZY, max_position=300),
+                    oracle_over=dict(summary_token=True, reindex_mode="lazy", max_position=300, max_chunk_span=wl.chunk_tokens))
+    assert all(r.get("summary_layers") == 1 for r in reps)
+    pos = hb.hermes_get_cache(ls.h, 0, 3)["pos"].cpu().numpy()[0]
+    assert (np.diff(pos) > 0).all() and pos.max() < 300
+    ls.close()
+    wl = CONFIGS["llava_ov_7b"].scaled(n_layers=7, budget=784, probe_tokens=64)    # bf16, tcgen05, V mover riding
+    mp = 784 + 197 * 4
+    _raw_steps_vs_lockstep(wl, 6, over=dict(summary_token=1, reindex_mode=hb.HERMES_REINDEX_LAZY, max_position=mp),
+                           oover=dict(summary_token=True, reindex_mode="lazy", max_position=mp, max_chunk_span=wl.chunk_tokens))
 
 
 def test_summary_token_with_16_frame_chunk():
