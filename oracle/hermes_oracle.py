@@ -42,7 +42,7 @@ __all__ = [
     "lambda_of_layer", "attention_weights", "recency_scores", "normalise_attention",
     "raw_scores", "smooth_scores", "select_topk", "compact_positions",
     "rope_frequencies", "pair_axis", "rotary_delta", "round_to_storage", "oracle_step",
-    "summary_token", "lazy_reindex_due",
+    "summary_token", "lazy_reindex_due", "layer_budgets", "smooth_scores_aligned", "oracle_step_layer_budgets",
 ]
 
 
@@ -81,6 +81,8 @@ class OracleConfig:
     probe_deep_begin: int = 0         # deep layers use probe rows [begin, P): the global prompt only (DESIGN f3)
     summary_token: bool = False       # deep layers: evicted tokens -> one summary token (Alg. 1; DESIGN f1)
     capacity: int = 0                 # slots per layer; 0 -> budget + largest chunk seen
+    budget_weights: tuple = (1.0, 1.0, 1.0)   # layer-dependent budgets: weight of a shallow / middle / deep layer
+                                      # (Tab. 5; DESIGN f4); equal weights = `budget` everywhere
 
     @property
     def n_axes(self) -> int:
@@ -324,6 +326,45 @@ def summary_token(cfg: OracleConfig, K_p: np.ndarray, V_p: np.ndarray, P_p: np.n
     return k_sum, v_sum
 
 
+# --------------------------------------------------------------------------- layer-dependent budgets (f4)
+def layer_budgets(cfg: OracleConfig) -> np.ndarray:
+    """Per-layer budgets m_i: with the total budget |M| = budget * L fixed,
+    m_i = floor(w_i / sum_j w_j * |M|), and the rounding residue |M| - sum_i m_i goes to the last layer.
+    w_i is the weight of layer i's stage (Tab. 5 gives one weight per stage).  The weights cross the C ABI
+    as single-precision numbers, so they are rounded to fp32 first; the quotient is taken in fp64."""
+    L = cfg.n_layers
+    w3 = [float(np.float32(x)) for x in cfg.budget_weights]
+    if min(w3) <= 0.0:
+        raise ValueError("budget weights must be positive")
+    stage_w = {"shallow": w3[0], "middle": w3[1], "deep": w3[2]}
+    w = np.array([stage_w[layer_stage(cfg, l)] for l in range(L)], np.float64)
+    total = cfg.budget * L
+    wsum = 0.0
+    for x in w:                                           # plain left-to-right fp64 sum (the host code does the same)
+        wsum += float(x)
+    m = np.array([int(np.floor(float(x) / wsum * float(total))) for x in w], np.int64)
+    m[L - 1] += total - int(m.sum())
+    return m
+
+
+def smooth_scores_aligned(cfg: OracleConfig, S: list) -> list:
+    """Eq. 5 when layers hold different numbers of candidates (DESIGN f4): the caches are aligned at
+    their NEWEST token -- candidate i of layer l (T_l candidates) meets candidate i - T_l + T_{l+1} of layer l+1, the
+    one at the same distance from the newest token, which both layers received together.  A candidate of layer l that
+    is older than everything layer l+1 holds has no counterpart and keeps its raw score.  With equal T this is
+    `smooth_scores`."""
+    L = len(S)
+    out = [np.array(x, dtype=np.float64, copy=True) for x in S]
+    for l in range(L - 1):
+        lam = lambda_of_layer(cfg, l)
+        T0, T1 = len(S[l]), len(S[l + 1])
+        i = np.arange(T0)
+        j = i - T0 + T1
+        has = j >= 0
+        out[l][has] = (1.0 - lam) * S[l][has] + lam * S[l + 1][j[has]]
+    return out
+
+
 # --------------------------------------------------------------------------- state + step
 @dataclass
 class OracleStream:
@@ -334,6 +375,7 @@ class OracleStream:
     V: Optional[np.ndarray] = None
     pos: Optional[np.ndarray] = None
     len: int = 0
+    lens: Optional[np.ndarray] = None # layer-dependent budgets (DESIGN f4): valid tokens per layer; `len` is then their max
     t_steps_seen: int = 0             # M-RoPE: temporal steps appended so far
     next_pos: int = -1                # lazy mode: position (1D) / temporal index (M-RoPE) after the newest token
     last: dict = field(default_factory=dict)
@@ -473,4 +515,74 @@ def oracle_step(st: OracleStream, K_new: np.ndarray, V_new: np.ndarray,
         st.next_pos = p_end + summ_pos
     st.last = {"T": T, "evicted": True, "reindexed": reindex, "W": W, "S": S, "S_tilde": S_tilde,
                "kept": kept, "pos_new": pos_new}
+    return st.last
+
+
+def oracle_step_layer_budgets(st: OracleStream, K_new: np.ndarray, V_new: np.ndarray,
+                              Q_probe: Optional[np.ndarray], pos_start: int = -1) -> dict:
+    """One chunk arrival with layer-dependent budgets (Tab. 5; DESIGN f4).
+
+    Every layer l has its own budget m_l (`layer_budgets`) and its own length len_l; it compresses -- Eq. 1-6, 8-10 as
+    in `oracle_step` -- only at an arrival that takes IT over its budget, and is left untouched (appended
+    to, not re-indexed) otherwise.  Arrival positions are shared by all layers and lie above every cached position:
+    1D default offset + max_l len_l.  Scores of layer l are taken over its own T_l = len_l + n_new candidates, the
+    recency term counts the distance from ITS newest token, and Eq. 5 pairs candidates at equal distance from the
+    newest token (`smooth_scores_aligned`).  1D RoPE, no summary token.  With equal weights this is `oracle_step`."""
+    cfg = st.cfg
+    if cfg.rope_mode != "1d" or cfg.summary_token:
+        raise ValueError("layer-dependent budgets are defined here for 1D RoPE without summary tokens (DESIGN f4)")
+    L, n_new = K_new.shape[0], K_new.shape[1]
+    m = layer_budgets(cfg)
+    if st.lens is None:
+        st.lens = np.zeros(L, np.int64)
+    lens = st.lens
+    T = lens + n_new
+    st.len = int(lens.max())
+    st._ensure(int(T.max()))
+    p_arr = arrival_positions(cfg, st, n_new, pos_start)
+    for l in range(L):
+        st.K[l, lens[l]:T[l]] = K_new[l]
+        st.V[l, lens[l]:T[l]] = V_new[l]
+        st.pos[l, :, lens[l]:T[l]] = p_arr
+    p_end = int(p_arr[0, 0]) + n_new
+    st.next_pos = p_end
+    over = T > m
+    if Q_probe is None or not over.any():
+        st.lens = T
+        st.len = int(T.max())
+        st.last = {"T": T.copy(), "evicted": False}
+        return st.last
+    scale = cfg.softmax_scale if cfg.softmax_scale > 0 else 1.0 / np.sqrt(float(cfg.head_dim))
+    S = []
+    for l in range(L):
+        R = recency_scores(int(T[l]), cfg.forget_rate, cfg.norm_mode)
+        if layer_stage(cfg, l) == "shallow":
+            S.append(R)
+            continue
+        pb = cfg.probe_deep_begin if layer_stage(cfg, l) == "deep" else 0
+        W = attention_weights(Q_probe[l][:, pb:], st.K[l, :T[l]], cfg.group, scale)
+        w = omega_of_layer(cfg, l)
+        S.append((1.0 - w) * normalise_attention(W, cfg.norm_mode) + w * R)
+    S_tilde = smooth_scores_aligned(cfg, S)
+    reindex = cfg.reindex_mode == "eager" or lazy_reindex_due(cfg, p_end)
+    kept, pos_new = [], []
+    new_lens = T.copy()
+    for l in range(L):
+        if not over[l]:                                   # under its budget: nothing happens to this layer
+            kept.append(np.arange(T[l])); pos_new.append(st.pos[l][:, :T[l]].copy())
+            continue
+        I = select_topk(S_tilde[l], int(m[l]))
+        p_old = st.pos[l][:, I]
+        p_new = compact_positions(cfg, p_old) if reindex else p_old
+        st.V[l, :m[l]] = st.V[l, I]
+        st.K[l, :m[l]] = rotary_delta(cfg, st.K[l, I], p_new - p_old)
+        st.pos[l, :, :m[l]] = p_new
+        kept.append(I); pos_new.append(p_new)
+        new_lens[l] = m[l]
+    st.lens = new_lens
+    st.len = int(new_lens.max())
+    if reindex:                                           # positions of the layers that compressed are below offset + m_l
+        st.next_pos = max(cfg.pos_offset + int(new_lens.max()), p_end if (~over).any() else 0)
+    st.last = {"T": T.copy(), "evicted": True, "evicted_layers": over.copy(), "reindexed": reindex, "S": S,
+               "S_tilde": S_tilde, "kept": kept, "pos_new": pos_new, "budgets": m}
     return st.last
