@@ -94,6 +94,11 @@ typedef struct {
                                    last_kept[budget-1] = -1 marks it.  Its position: pos_offset+budget-1 at a step that
                                    re-indexes; under LAZY re-indexing, between re-index steps, the position after the
                                    newest token (the next chunk then starts one position later).  Needs HERMES_ROPE_1D  */
+  float budget_weight[3];       /* layer-dependent budgets (Tab. 5): weight of a shallow / middle / deep
+                                   layer.  With the total budget * n_layers fixed, layer i keeps
+                                   m_i = floor(w_i / sum_j w_j * budget * n_layers) tokens, the residue goes to the last
+                                   layer.  {1, 1, 1} (default): `budget` everywhere.  Unequal weights need HERMES_ROPE_1D,
+                                   no summary token, and score on the CUDA-core path                              */
   int32_t defer_v;              /* 1 (default): on the tcgen05 path an eviction compacts K at once but leaves the
                                    kept V rows to be moved by the NEXT update's scoring kernel (V is not read by
                                    scoring, so the copy hides behind it); hermes_get_cache() and updates that do
@@ -110,10 +115,10 @@ typedef struct {
   const int32_t *pos;           /* [n_axes][pos_stride]; first `len` entries of each axis valid */
   int32_t n_axes;               /* 1 (1D RoPE) or 3 (M-RoPE: t, h, w)                          */
   int32_t pos_stride;
-  int32_t len;                  /* host-tracked: min(tokens appended, budget) after an eviction */
+  int32_t len;                  /* host-tracked: min(tokens appended, this layer's budget) after an eviction */
   const float *last_scores;     /* [last_T] smoothed scores S~ of the last eviction, else NULL  */
-  const int32_t *last_kept;     /* [budget] ascending indices I_l into the last candidate list  */
-  int32_t last_T;               /* candidates of the last eviction (0 if none yet)              */
+  const int32_t *last_kept;     /* [len] ascending indices I_l into the last candidate list      */
+  int32_t last_T;               /* this layer's candidates at the last eviction (0 if none yet)  */
 } hermes_cache_view;
 
 /* Defaults of the paper for everything but geometry; geometry fields are 0. */
@@ -141,12 +146,13 @@ int hermes_create(const hermes_config *cfg, void *workspace, size_t bytes, herme
 int hermes_append_chunk(hermes_t *h, const void *K_new, const void *V_new, const void *Q_probe,
                         int32_t n_new, int32_t n_probe, int32_t pos_start, void *cuda_stream);
 
-/* Same update with HOST buffers (pinned memory recommended): stages Q_probe and K_new to the device with
- * cudaMemcpyAsync on `cuda_stream`, V_new on a library-owned side stream (created on first use) so that its
- * copy overlaps the scoring kernels, which never read V; the V rows are appended behind an event wait on
- * `cuda_stream`, so everything the call enqueues is ordered on `cuda_stream` when it returns.  If
- * kept_out != NULL, copies the kept index lists I_l [B, L, budget] int32 back to the host (only meaningful
- * when an eviction ran).  The host buffers must stay valid until `cuda_stream` has passed the call.          */
+/* Same update with HOST buffers (pinned memory recommended), which must hold their data when the call is made: Q_probe,
+ * K_new and then V_new are copied to the device with cudaMemcpyAsync on a library-owned copy stream (created on first
+ * use) into one of two staging sets, so the copies of a call overlap the kernels of the call before it; `cuda_stream`
+ * waits for K before the update's kernels and for V before the V rows are appended, so everything the call enqueues is
+ * ordered on `cuda_stream` when it returns.  If kept_out != NULL, copies the kept index lists I_l [B, L, budget] int32
+ * back to the host on `cuda_stream` (only meaningful when an eviction ran; not available with layer-dependent budgets).
+ * The host buffers must stay valid until `cuda_stream` has passed the call.                                           */
 int hermes_append_chunk_host(hermes_t *h, const void *K_new_host, const void *V_new_host,
                              const void *Q_probe_host, int32_t n_new, int32_t n_probe,
                              int32_t pos_start, int32_t *kept_out_host, void *cuda_stream);
@@ -155,8 +161,14 @@ int hermes_append_chunk_host(hermes_t *h, const void *K_new_host, const void *V_
  * on the stream of the last append first.                                                              */
 int hermes_get_cache(hermes_t *h, int32_t stream, int32_t layer, hermes_cache_view *out);
 
-/* Host-tracked token count per layer (same for every stream and layer).                              */
+/* Host-tracked token count per layer (same for every stream; with layer-dependent budgets the largest layer's). */
 int32_t hermes_len(const hermes_t *h);
+
+/* Host-tracked token count of one layer (differs from hermes_len only with layer-dependent budgets); -1 if out of range. */
+int32_t hermes_layer_len(const hermes_t *h, int32_t layer);
+
+/* Budget m_i of one layer (hermes_config.budget unless budget_weight is unequal); -1 if out of range.            */
+int32_t hermes_layer_budget(const hermes_t *h, int32_t layer);
 
 /* Device-side sticky status word, read with a blocking copy: 0 = ok; bit0 = M-RoPE coordinate range
  * too wide to compact, bit1 = rotary delta outside the table (slow path taken; results still valid).  */

@@ -21,7 +21,7 @@ HERMES_SCORE_AUTO, HERMES_SCORE_SIMT, HERMES_SCORE_TCGEN05 = 0, 1, 2
 HERMES_K_NAMES = ("append", "score_stats", "score_combine", "score_colsum", "select", "gather", "summary")
 
 EXPORTS = ("hermes_default_config", "hermes_workspace_bytes", "hermes_create", "hermes_append_chunk",
-           "hermes_append_chunk_host", "hermes_get_cache", "hermes_len", "hermes_device_status",
+           "hermes_append_chunk_host", "hermes_get_cache", "hermes_len", "hermes_layer_len", "hermes_layer_budget", "hermes_device_status",
            "hermes_set_profiling", "hermes_get_profile", "hermes_last_score_path", "hermes_v_pending",
            "hermes_last_launch_count", "hermes_destroy", "hermes_last_error")
 
@@ -37,7 +37,7 @@ class HermesConfig(C.Structure):
                 ("rope_theta", C.c_float), ("mrope_section", C.c_int32 * 3),
                 ("mrope_compact_axes", C.c_int32), ("mrope_grid_h", C.c_int32),
                 ("mrope_grid_w", C.c_int32), ("pos_offset", C.c_int32), ("reindex_mode", C.c_int32),
-                ("max_position", C.c_int32), ("probe_deep_begin", C.c_int32), ("summary_token", C.c_int32), ("defer_v", C.c_int32), ("score_path", C.c_int32),
+                ("max_position", C.c_int32), ("probe_deep_begin", C.c_int32), ("summary_token", C.c_int32), ("budget_weight", C.c_float * 3), ("defer_v", C.c_int32), ("score_path", C.c_int32),
                 ("device", C.c_int32)]
 
 
@@ -77,6 +77,8 @@ def load_library(rebuild_if_stale: bool = True) -> C.CDLL:
     lib.hermes_append_chunk_host.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp]
     lib.hermes_get_cache.argtypes = [vp, i32, i32, C.POINTER(HermesCacheView)]
     lib.hermes_len.argtypes = [vp]
+    lib.hermes_layer_len.argtypes = [vp, i32]
+    lib.hermes_layer_budget.argtypes = [vp, i32]
     lib.hermes_device_status.argtypes = [vp, C.POINTER(i32)]
     lib.hermes_set_profiling.argtypes = [vp, i32]
     lib.hermes_get_profile.argtypes = [vp, C.POINTER(C.c_float), i32]
@@ -98,6 +100,8 @@ def hermes_default_config(**kw) -> HermesConfig:
     for k, v in kw.items():
         if k == "mrope_section":
             cfg.mrope_section = (C.c_int32 * 3)(*v)
+        elif k == "budget_weight":
+            cfg.budget_weight = (C.c_float * 3)(*v)
         elif not hasattr(cfg, k):
             raise TypeError(f"hermes_config has no field {k!r}")
         else:
@@ -216,12 +220,20 @@ def hermes_get_cache(h: Handle, stream: int, layer: int) -> dict:
     out["pos"] = pos[:, :v.len]
     if v.last_T:
         out["last_scores"] = _view(h, v.last_scores, v.last_T * 4, torch.float32, (v.last_T,))
-        out["last_kept"] = _view(h, v.last_kept, c.budget * 4, torch.int32, (c.budget,))
+        out["last_kept"] = _view(h, v.last_kept, v.len * 4, torch.int32, (v.len,))
     return out
 
 
 def hermes_len(h: Handle) -> int:
     return int(load_library().hermes_len(h.ptr))
+
+
+def hermes_layer_len(h: Handle, layer: int) -> int:
+    return int(load_library().hermes_layer_len(h.ptr, layer))
+
+
+def hermes_layer_budget(h: Handle, layer: int) -> int:
+    return int(load_library().hermes_layer_budget(h.ptr, layer))
 
 
 def hermes_device_status(h: Handle) -> int:

@@ -49,7 +49,14 @@ struct Geom {
   float* lambda;    // [L] Eq. 7
   int32_t* status;  // sticky device status word
   unsigned* seg_cnt;// [B*L*n_vh_max] tcgen05 scoring: pass-1 progress per group, zeroed by k_append
+  // layer-dependent budgets (DESIGN f4); both NULL otherwise.  Rewritten by a stream-ordered copy before every update.
+  const int32_t* lay_T;    // [L] candidates T_l = len_l + n_new of this update
+  const int32_t* lay_keep; // [L] tokens layer l holds after this update: m_l if T_l > m_l (it compresses), else T_l
 };
+
+// Candidates / retained tokens of layer l in this update (uniform: the kernel's scalar arguments).
+__device__ __forceinline__ int layer_T(const Geom& g, int l, int Tn) { return g.lay_T ? __ldg(g.lay_T + l) : Tn; }
+__device__ __forceinline__ int layer_keep(const Geom& g, int l) { return g.lay_keep ? __ldg(g.lay_keep + l) : g.budget; }
 
 __host__ __device__ inline size_t slab_index(const Geom& g, int b, int l, int buf) {
   return (size_t(b) * g.L + l) * 2 + buf;

@@ -51,6 +51,7 @@ extern "C" void hermes_default_config(hermes_config* c) {
   c->score_path = HERMES_SCORE_AUTO;
   c->reindex_mode = HERMES_REINDEX_EAGER;
   c->defer_v = 1;
+  c->budget_weight[0] = c->budget_weight[1] = c->budget_weight[2] = 1.f;
 }
 
 extern "C" size_t hermes_workspace_bytes(const hermes_config* c) {
@@ -60,6 +61,14 @@ extern "C" size_t hermes_workspace_bytes(const hermes_config* c) {
 
 extern "C" const char* hermes_last_error(const hermes_t* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 extern "C" int32_t hermes_len(const hermes_t* h) { return h ? h->len : 0; }
+extern "C" int32_t hermes_layer_len(const hermes_t* h, int32_t layer) {
+  if (!h || layer < 0 || layer >= h->cfg.n_layers) return -1;
+  return h->lb ? h->lay_len[layer] : h->len;
+}
+extern "C" int32_t hermes_layer_budget(const hermes_t* h, int32_t layer) {
+  if (!h || layer < 0 || layer >= h->cfg.n_layers) return -1;
+  return h->lay_budget[layer];
+}
 extern "C" int32_t hermes_last_score_path(const hermes_t* h) { return h ? h->last_score_path : 0; }
 extern "C" int32_t hermes_v_pending(const hermes_t* h) { return h && h->v_pending ? 1 : 0; }
 extern "C" int32_t hermes_last_launch_count(const hermes_t* h) { return h ? h->last_launches : 0; }
@@ -85,7 +94,7 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   {
     cudaFuncAttributes fa;
     CUDA_TRY(nullptr, cudaFuncGetAttributes(&fa, k_select));
-    if (fa.sharedSizeBytes + size_t(y.cap) * 4 > prop.sharedMemPerBlockOptin)
+    if (fa.sharedSizeBytes + size_t(sel_quarter(y.cap)) * 4 > prop.sharedMemPerBlockOptin)
       return fail(nullptr, HERMES_EINVAL, "max_tokens %d too large for the select kernel's shared memory", y.cap);
     if (c->summary_token) {
       const size_t need = size_t(y.cap - c->budget + 2) * 8;
@@ -109,7 +118,14 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   Geom& g = h->geom;
   g.B = c->n_streams; g.L = c->n_layers; g.Hq = c->n_q_heads; g.Hkv = c->n_kv_heads;
   g.G = c->n_q_heads / c->n_kv_heads; g.d = c->head_dim;
-  g.cap = y.cap; g.budget = c->budget; g.n_axes = y.n_axes; g.row_elems = c->n_kv_heads * c->head_dim;
+  // layer-dependent budgets: g.budget is the stride of the kept / delta lists (the largest layer budget); the per-layer
+  // counts come from lay_T / lay_keep, rewritten before every update
+  h->lb = !uniform_budgets(*c);
+  h->lay_budget = layer_budgets(*c, y.n_shallow, y.n_deep);
+  h->lay_len.assign(c->n_layers, 0); h->lay_last_T.assign(c->n_layers, 0);
+  g.cap = y.cap; g.budget = y.budget_max; g.n_axes = y.n_axes; g.row_elems = c->n_kv_heads * c->head_dim;
+  g.lay_T = h->lb ? reinterpret_cast<const int32_t*>(h->ws + y.lay_dyn) : nullptr;
+  g.lay_keep = h->lb ? g.lay_T + c->n_layers : nullptr;
   g.n_shallow = y.n_shallow; g.n_deep = y.n_deep; g.summary = c->summary_token; g.probe_deep_begin = c->probe_deep_begin; g.n_evict_max = y.cap - c->budget + 1;
   g.p_max = c->max_probe_tokens; g.pos_offset = c->pos_offset;
   g.sec_t = c->mrope_section[0]; g.sec_h = c->mrope_section[1];
@@ -174,7 +190,7 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   if (e == cudaSuccess) e = cudaMemset(g.status, 0, 256);
   if (e == cudaSuccess) e = cudaMemset(h->ws + y.seg_cnt, 0, size_t(g.B) * L * y.n_vh_max * 4);
   if (e == cudaSuccess) e = cudaMemset(g.posc, 0, size_t(g.B) * L * 2 * y.n_axes * y.cap * 4);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_select, cudaFuncAttributeMaxDynamicSharedMemorySize, y.cap * 4);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_select, cudaFuncAttributeMaxDynamicSharedMemorySize, sel_quarter(y.cap) * 4);
   if (e == cudaSuccess) e = cudaDeviceSynchronize();
   if (e != cudaSuccess) {
     fail(nullptr, HERMES_ECUDA, "create: %s", cudaGetErrorString(e));
@@ -182,7 +198,7 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
     return HERMES_ECUDA;
   }
   // tensor-core scoring path: bf16, d = 128; probing it builds its tensor maps
-  h->tc_ok = tc_init(h);
+  h->tc_ok = !h->lb && tc_init(h);                 // layer-dependent budgets score on the CUDA-core path
   if (c->score_path == HERMES_SCORE_TCGEN05 && !h->tc_ok) {
     std::string why = h->err;
     delete h;
@@ -196,7 +212,10 @@ extern "C" void hermes_destroy(hermes_t* h) {
   if (!h) return;
   if (h->timer.created)
     for (int i = 0; i < HERMES_K_COUNT; ++i) { cudaEventDestroy(h->timer.beg[i]); cudaEventDestroy(h->timer.end[i]); }
-  if (h->side_stream) { cudaStreamSynchronize(h->side_stream); cudaStreamDestroy(h->side_stream); cudaEventDestroy(h->ev_k_done); cudaEventDestroy(h->ev_v_done); }
+  if (h->side_stream) {
+    cudaStreamSynchronize(h->side_stream); cudaStreamDestroy(h->side_stream);
+    for (int p = 0; p < 2; ++p) { cudaEventDestroy(h->ev_k_done[p]); cudaEventDestroy(h->ev_v_done[p]); cudaEventDestroy(h->ev_free[p]); }
+  }
   tc_destroy(h);
   delete h;
 }
@@ -247,8 +266,8 @@ extern "C" int hermes_get_cache(hermes_t* h, int32_t stream, int32_t layer, herm
   out->k = static_cast<char*>(g.kc) + slab * g.cap * h->lay.row_bytes;
   out->v = static_cast<char*>(g.vc) + slab * g.cap * h->lay.row_bytes;
   out->pos = g.posc + slab * g.n_axes * g.cap;
-  out->n_axes = g.n_axes; out->pos_stride = g.cap; out->len = h->len;
-  out->last_T = h->last_T;
+  out->n_axes = g.n_axes; out->pos_stride = g.cap; out->len = h->lb ? h->lay_len[layer] : h->len;
+  out->last_T = h->lb ? h->lay_last_T[layer] : h->last_T;
   out->last_scores = h->last_T ? g.scores + bl * g.cap : nullptr;
   out->last_kept = h->last_T ? g.kept + bl * g.budget : nullptr;
   return HERMES_OK;
@@ -335,7 +354,7 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
   if (n_new <= 0) return fail(h, HERMES_EINVAL, "n_new = %d must be positive", n_new);
   if (Q_probe && (n_probe <= 0 || n_probe > c.max_probe_tokens)) return fail(h, HERMES_EINVAL, "n_probe = %d not in [1, %d]", n_probe, c.max_probe_tokens);
   if (Q_probe && c.probe_deep_begin >= n_probe) return fail(h, HERMES_EINVAL, "probe_deep_begin %d leaves no probe row of %d for the deep layers", c.probe_deep_begin, n_probe);
-  const int Tn = h->len + n_new;
+  const int Tn = h->len + n_new;                  // layer-dependent budgets: the largest layer's candidates
   if (Tn > g.cap) return fail(h, HERMES_ECAPACITY, "len %d + n_new %d exceeds max_tokens %d", h->len, n_new, g.cap);
   // arrival positions (DESIGN c16): host-computable, strictly above every cached position
   long long p0;
@@ -352,7 +371,18 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
   }
   if (p0 < h->next_pos) return fail(h, HERMES_EINVAL, "pos_start %lld is not above the cached positions (need >= %lld)", p0, h->next_pos);
   if (p0 + std::max<long long>(n_new, steps) >= INT_MAX) return fail(h, HERMES_EINVAL, "position overflow");
-  const bool evict = Q_probe != nullptr && Tn > c.budget;
+  bool evict = Q_probe != nullptr && Tn > c.budget;
+  std::vector<int32_t> dyn;                       // layer-dependent budgets: [T_l | tokens held after this update]
+  if (h->lb) {
+    dyn.resize(2 * size_t(c.n_layers));
+    evict = false;
+    for (int l = 0; l < c.n_layers; ++l) {
+      const int T_l = h->lay_len[l] + n_new;
+      const bool over = Q_probe != nullptr && T_l > h->lay_budget[l];   // a layer compresses when IT exceeds its budget
+      dyn[l] = T_l; dyn[c.n_layers + l] = over ? h->lay_budget[l] : T_l;
+      evict |= over;
+    }
+  }
   // the lazy re-index trigger reasons about "the next chunk" with max_chunk_tokens; elsewhere only the capacity binds
   if (lazy && evict && n_new > c.max_chunk_tokens)
     return fail(h, HERMES_EINVAL, "n_new = %d exceeds max_chunk_tokens %d (lazy re-indexing)", n_new, c.max_chunk_tokens);
@@ -365,6 +395,8 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
   if (lazy && p0 + span > c.max_position) return fail(h, HERMES_ECAPACITY, "positions would exceed max_position %d", c.max_position);
 
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  // stream-ordered behind the previous update's kernels; the source is pageable memory, so the call has staged it on return
+  if (h->lb) CUDA_TRY(h, cudaMemcpyAsync(h->ws + h->lay.lay_dyn, dyn.data(), dyn.size() * 4, cudaMemcpyHostToDevice, s));
   h->last_launches = 0;
   for (bool& r : h->timer.ran) r = false;
   const int row_vecs = int(h->lay.row_bytes / 16);
@@ -416,7 +448,7 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
       const float r_norm_sum = float((1.0 - std::exp(-k)) / (1.0 - std::exp(-k * Tn)));
       if (g.L > g.n_shallow)
         launch_pdl(k_wsum, dim3((Tn + 255) / 256, g.B * (g.L - g.n_shallow)), dim3(256), 0, s, g, Tn, n_probe, h->n_vh);
-      launch_pdl(k_select, dim3(BL), dim3(kSelThreads), size_t(Tn) * 4, s, g, h->cur, Tn, c.forget_rate, int(c.norm_mode == HERMES_NORM_SUM), r_norm_sum, int(reindex),
+      launch_pdl(k_select, dim3(BL * kSelCluster), dim3(kSelThreads), size_t(sel_quarter(Tn)) * 4, s, g, h->cur, Tn, c.forget_rate, int(c.norm_mode == HERMES_NORM_SUM), r_norm_sum, int(reindex),
                  reindex ? c.pos_offset + c.budget - 1 : int(p0 + span));
     }
     if (c.summary_token && h->lay.n_deep > 0) {
@@ -441,7 +473,20 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
   if (e != cudaSuccess) return fail(h, HERMES_ECUDA, "kernel launch failed: %s", cudaGetErrorString(e));
   // commit host-tracked state
   if (g.n_axes == 3) h->t_steps_seen += steps;
-  if (evict) {
+  if (h->lb) {
+    int mx = 0;
+    bool untouched = false;                         // a layer under its budget keeps its original positions
+    for (int l = 0; l < c.n_layers; ++l) {
+      if (evict) h->lay_last_T[l] = dyn[l];
+      h->lay_len[l] = evict ? dyn[c.n_layers + l] : dyn[l];
+      untouched |= dyn[c.n_layers + l] == dyn[l];
+      mx = std::max(mx, h->lay_len[l]);
+    }
+    if (evict) { h->cur ^= 1; h->last_T = Tn; }
+    h->len = mx;
+    // after a re-index step every position of a layer that compressed is below offset + m_l (DESIGN f4)
+    h->next_pos = (!evict || !reindex) ? p0 + n_new : std::max<long long>(c.pos_offset + mx, untouched ? p0 + n_new : 0);
+  } else if (evict) {
     h->cur ^= 1; h->len = c.budget; h->last_T = Tn;
     if (!reindex) h->next_pos = p0 + span + summ_pos; else
     // after eager re-indexing every cached position is below offset + budget (1D) or below
@@ -466,31 +511,43 @@ extern "C" int hermes_append_chunk_host(hermes_t* h, const void* K_host, const v
   if (!K_host || !V_host) return fail(h, HERMES_EINVAL, "K_new / V_new must not be NULL");
   const hermes_config& c = h->cfg;
   if (n_new <= 0 || n_new > c.max_chunk_tokens) return fail(h, HERMES_EINVAL, "n_new = %d not in [1, %d] (host path)", n_new, c.max_chunk_tokens);
+  if (h->lb && kept_out_host) return fail(h, HERMES_EINVAL, "kept_out is not available with layer-dependent budgets (use hermes_get_cache)");
   if (Q_host && (n_probe <= 0 || n_probe > c.max_probe_tokens)) return fail(h, HERMES_EINVAL, "n_probe = %d not in [1, %d]", n_probe, c.max_probe_tokens);
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   const size_t BL = size_t(c.n_streams) * c.n_layers;
   const size_t kv_bytes = BL * n_new * h->lay.row_bytes;
-  char* sk = h->ws + h->lay.stage_k; char* sv = h->ws + h->lay.stage_v; char* sq = h->ws + h->lay.stage_q;
-  // Q and K go first on the caller's stream; V follows on a side stream once K is across, so that it moves while
-  // the scoring kernels (which never read V) run.  The event after the K copy also orders the side stream behind
-  // every earlier reader of the V staging buffer.
+  // Two staging sets: the copies of this call run on the library's copy stream while the kernels of the previous call (on
+  // the caller's stream) still read the other set.  Q and K go first, V last: the scoring kernels, which never read V,
+  // start as soon as K is across, and the V rows are appended behind an event wait.
+  const int p = int(h->host_calls & 1u);
+  char* sk = h->ws + h->lay.stage_k + p * h->lay.stage_kv_bytes;
+  char* sv = h->ws + h->lay.stage_v + p * h->lay.stage_kv_bytes;
+  char* sq = h->ws + h->lay.stage_q + p * h->lay.stage_q_bytes;
   if (!h->side_stream) {
     CUDA_TRY(h, cudaStreamCreateWithFlags(&h->side_stream, cudaStreamNonBlocking));
-    CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_k_done, cudaEventDisableTiming));
-    CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_v_done, cudaEventDisableTiming));
+    for (int i = 0; i < 2; ++i) {
+      CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_k_done[i], cudaEventDisableTiming));
+      CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_v_done[i], cudaEventDisableTiming));
+      CUDA_TRY(h, cudaEventCreateWithFlags(&h->ev_free[i], cudaEventDisableTiming));
+    }
   }
-  if (Q_host) CUDA_TRY(h, cudaMemcpyAsync(sq, Q_host, BL * c.n_q_heads * n_probe * c.head_dim * h->lay.esize, cudaMemcpyHostToDevice, s));
-  CUDA_TRY(h, cudaMemcpyAsync(sk, K_host, kv_bytes, cudaMemcpyHostToDevice, s));
-  CUDA_TRY(h, cudaEventRecord(h->ev_k_done, s));
-  CUDA_TRY(h, cudaStreamWaitEvent(h->side_stream, h->ev_k_done, 0));
-  CUDA_TRY(h, cudaMemcpyAsync(sv, V_host, kv_bytes, cudaMemcpyHostToDevice, h->side_stream));
-  CUDA_TRY(h, cudaEventRecord(h->ev_v_done, h->side_stream));
+  cudaStream_t cs = h->side_stream;
+  if (h->ev_free_set[p]) CUDA_TRY(h, cudaStreamWaitEvent(cs, h->ev_free[p], 0));   // the call before the last is done with set p
+  if (Q_host) CUDA_TRY(h, cudaMemcpyAsync(sq, Q_host, BL * c.n_q_heads * n_probe * c.head_dim * h->lay.esize, cudaMemcpyHostToDevice, cs));
+  CUDA_TRY(h, cudaMemcpyAsync(sk, K_host, kv_bytes, cudaMemcpyHostToDevice, cs));
+  CUDA_TRY(h, cudaEventRecord(h->ev_k_done[p], cs));
+  CUDA_TRY(h, cudaMemcpyAsync(sv, V_host, kv_bytes, cudaMemcpyHostToDevice, cs));
+  CUDA_TRY(h, cudaEventRecord(h->ev_v_done[p], cs));
+  CUDA_TRY(h, cudaStreamWaitEvent(s, h->ev_k_done[p], 0));
+  ++h->host_calls;
   const int len_before = h->len;
-  int rc = append_impl(h, sk, sv, Q_host ? sq : nullptr, n_new, n_probe, pos_start, cuda_stream, h->ev_v_done);
-  if (rc != HERMES_OK) {                               // nothing was enqueued: still join the side stream
-    cudaStreamWaitEvent(s, h->ev_v_done, 0);
+  int rc = append_impl(h, sk, sv, Q_host ? sq : nullptr, n_new, n_probe, pos_start, cuda_stream, h->ev_v_done[p]);
+  if (rc != HERMES_OK) {                               // nothing was enqueued: still join the copy stream
+    cudaStreamWaitEvent(s, h->ev_v_done[p], 0);
     return rc;
   }
+  CUDA_TRY(h, cudaEventRecord(h->ev_free[p], s));
+  h->ev_free_set[p] = true;
   const bool evicted = Q_host && len_before + n_new > c.budget;
   if (kept_out_host && evicted)
     CUDA_TRY(h, cudaMemcpyAsync(kept_out_host, h->geom.kept, BL * c.budget * 4, cudaMemcpyDeviceToHost, s));

@@ -1,5 +1,6 @@
 // Host-side state of a handle: validated config, workspace carve-up, host-tracked stream state.
 #pragma once
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -17,10 +18,33 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {           // byte offsets into the workspace
   size_t kc, vc, posc, colsum, wsum, wmax, rowstat, partial, scores, kept, delta, evicted, rope_tab, rope_freq, sum_tab, omega, lambda,
-      status, seg_cnt, stage_k, stage_v, stage_q, tmaps, total;
+      status, seg_cnt, lay_dyn, stage_k, stage_v, stage_q, tmaps, total;
   int cap, n_axes, n_part_max, table_rows, n_shallow, n_middle, n_deep, n_vh_max, sum_tab_neg, sum_tab_rows;
-  size_t esize, row_bytes;
+  int budget_max, budget_min;   // largest / smallest layer budget (= budget unless budget_weight is unequal)
+  size_t esize, row_bytes, stage_kv_bytes, stage_q_bytes;
 };
+
+// Layer-dependent budgets: m_i = floor(w_i / sum_j w_j * budget * L), residue to the last layer; w_i is
+// the weight of layer i's stage.  Same arithmetic as the oracle: fp32 weights, left-to-right fp64 sum, fp64 quotient.
+inline bool uniform_budgets(const hermes_config& c) {
+  return c.budget_weight[0] == c.budget_weight[1] && c.budget_weight[1] == c.budget_weight[2];
+}
+inline std::vector<int> layer_budgets(const hermes_config& c, int n_shallow, int n_deep) {
+  const int L = c.n_layers;
+  std::vector<int> m(L, c.budget);
+  if (uniform_budgets(c)) return m;
+  std::vector<double> w(L);
+  double wsum = 0.0;
+  for (int l = 0; l < L; ++l) {
+    w[l] = double(l < n_shallow ? c.budget_weight[0] : l < L - n_deep ? c.budget_weight[1] : c.budget_weight[2]);
+    wsum += w[l];
+  }
+  const long long total = (long long)c.budget * L;
+  long long acc = 0;
+  for (int l = 0; l < L; ++l) { m[l] = int(std::floor(w[l] / wsum * double(total))); acc += m[l]; }
+  m[L - 1] += int(total - acc);
+  return m;
+}
 
 inline void stage_split(int L, int& n_shallow, int& n_deep) {   // PAPER.md:144; rounding DESIGN c7
   if (n_shallow < 0) n_shallow = std::max(1, (L + 5) / 10);
@@ -71,26 +95,37 @@ inline const char* validate(const hermes_config& c) {
     if (c.max_position > (1 << 20)) return "max_position too large (rotary table)";
   }
   if (c.score_path < HERMES_SCORE_AUTO || c.score_path > HERMES_SCORE_TCGEN05) return "bad score_path";
+  for (float w : c.budget_weight) if (!(w > 0.f) || !std::isfinite(w)) return "budget_weight must be positive";
+  if (!uniform_budgets(c)) {
+    if (c.rope_mode != HERMES_ROPE_1D || c.summary_token) return "layer-dependent budgets need 1D RoPE and no summary token";
+    if (c.score_path == HERMES_SCORE_TCGEN05) return "layer-dependent budgets score on the CUDA-core path";
+    for (int m : layer_budgets(c, ns, nd)) {
+      if (m < 1) return "a layer's budget would be zero";
+      if (c.max_tokens != 0 && c.max_tokens <= m) return "max_tokens must exceed the largest layer budget (or be 0)";
+    }
+  }
   if (size_t(c.budget) + size_t(c.max_chunk_tokens) > (size_t(1) << 24)) return "budget + chunk too large";
   return nullptr;
 }
 
 inline Layout make_layout(const hermes_config& c) {
   Layout y{};
-  y.cap = c.max_tokens ? c.max_tokens : c.budget + c.max_chunk_tokens;
+  int ns = c.n_shallow, nd = c.n_deep;
+  stage_split(c.n_layers, ns, nd);
+  y.n_shallow = ns; y.n_deep = nd; y.n_middle = c.n_layers - ns - nd;
+  y.budget_max = y.budget_min = c.budget;
+  for (int m : layer_budgets(c, ns, nd)) { y.budget_max = std::max(y.budget_max, m); y.budget_min = std::min(y.budget_min, m); }
+  y.cap = c.max_tokens ? c.max_tokens : y.budget_max + c.max_chunk_tokens;
   y.n_axes = c.rope_mode == HERMES_ROPE_M3D ? 3 : 1;
   y.esize = c.dtype == HERMES_BF16 ? 2 : 4;
   y.row_bytes = size_t(c.n_kv_heads) * c.head_dim * y.esize;
   y.n_part_max = (y.cap + 127) / 128;
   y.n_vh_max = 4 * c.n_kv_heads * std::max(1, (c.n_q_heads / c.n_kv_heads * c.max_probe_tokens + 511) / 512);
-  int ns = c.n_shallow, nd = c.n_deep;
-  stage_split(c.n_layers, ns, nd);
-  y.n_shallow = ns; y.n_deep = nd; y.n_middle = c.n_layers - ns - nd;
   if (c.rope_mode == HERMES_ROPE_M3D) {
     const int tpt = c.mrope_grid_h * c.mrope_grid_w;
     y.table_rows = c.budget + (c.max_chunk_tokens + tpt - 1) / tpt + 2;
   } else {
-    y.table_rows = y.cap - c.budget + 1 + (c.summary_token ? 1 : 0);   // summary layers evict one token more
+    y.table_rows = y.cap - y.budget_min + 1 + (c.summary_token ? 1 : 0);   // summary layers evict one token more
   }
   // lazy mode: a re-index step moves positions from anywhere below the limit down to the compact range
   if (c.reindex_mode == HERMES_REINDEX_LAZY) y.table_rows = std::max(y.table_rows, c.max_position - c.pos_offset + 2);
@@ -107,8 +142,8 @@ inline Layout make_layout(const hermes_config& c) {
   y.rowstat = take(BL * rows * 2 * 4);
   y.partial = take(BL * rows * y.n_part_max * 2 * 4);
   y.scores = take(BL * y.cap * 4);
-  y.kept = take(BL * c.budget * 4);
-  y.delta = take(BL * y.n_axes * c.budget * 4);
+  y.kept = take(BL * y.budget_max * 4);
+  y.delta = take(BL * y.n_axes * y.budget_max * 4);
   y.evicted = take(BL * size_t(y.cap - c.budget + 1) * 4);
   y.rope_tab = take(size_t(y.table_rows) * (c.head_dim / 2) * 8);
   y.rope_freq = take(size_t(c.head_dim / 2) * 8);
@@ -127,9 +162,13 @@ inline Layout make_layout(const hermes_config& c) {
   y.lambda = take(size_t(c.n_layers) * 4);
   y.status = take(256);
   y.seg_cnt = take(BL * y.n_vh_max * 4);
-  y.stage_k = take(BL * c.max_chunk_tokens * y.row_bytes);
-  y.stage_v = take(BL * c.max_chunk_tokens * y.row_bytes);
-  y.stage_q = take(BL * rows * c.head_dim * y.esize);
+  y.lay_dyn = take(size_t(c.n_layers) * 2 * 4);
+  // staging of the host entry point, two sets: the copies of call n + 1 run while the kernels of call n read set n & 1
+  y.stage_kv_bytes = align_up(BL * c.max_chunk_tokens * y.row_bytes);
+  y.stage_q_bytes = align_up(BL * rows * c.head_dim * y.esize);
+  y.stage_k = take(2 * y.stage_kv_bytes);
+  y.stage_v = take(2 * y.stage_kv_bytes);
+  y.stage_q = take(2 * y.stage_q_bytes);
   y.tmaps = take(4096);
   y.total = o;
   return y;
@@ -160,7 +199,9 @@ struct hermes {
   hk::Layout lay{};
   hk::Geom geom{};
   char* ws = nullptr;
-  int len = 0;              // tokens per layer (host-tracked; identical for all streams / layers)
+  int len = 0;              // tokens per layer (host-tracked; identical for all streams / layers; LB: the largest layer's)
+  bool lb = false;          // layer-dependent budgets (DESIGN f4)
+  std::vector<int> lay_budget, lay_len, lay_last_T;   // per layer: m_l, tokens held, candidates at the last eviction
   int cur = 0;              // which half of the double buffer is current
   long long t_steps_seen = 0;   // M-RoPE temporal steps appended so far
   long long next_pos = 0;   // smallest admissible pos_start of the next chunk
@@ -168,8 +209,12 @@ struct hermes {
   int last_score_path = 0;
   int last_launches = 0;
   int n_sm = 148;
-  cudaStream_t side_stream = nullptr;   // host entry point: V's host-to-device copy (created on first use)
-  cudaEvent_t ev_k_done = nullptr, ev_v_done = nullptr;
+  // host entry point: all host-to-device copies run on a library-owned copy stream (created on first use), into
+  // staging set (call count & 1); ev_free[p] = the kernels that read set p have been enqueued and executed
+  cudaStream_t side_stream = nullptr;
+  cudaEvent_t ev_k_done[2] = {nullptr, nullptr}, ev_v_done[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
+  bool ev_free_set[2] = {false, false};
+  unsigned host_calls = 0;
   int n_vh = 0;             // column-sum slots written by the last scoring pass
   // deferred V compaction: after an eviction on the tcgen05 path k_gather moves only K; the kept V rows still sit
   // in buffer v_src_buf and are moved into the current buffer by the NEXT update's scoring kernel (or by a flush)

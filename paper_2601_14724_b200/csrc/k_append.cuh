@@ -15,6 +15,7 @@ k_append(Geom g, const uint4* __restrict__ k_new, const uint4* __restrict__ v_ne
   pdl_wait();
   pdl_launch_dependents();
   const int bl = blockIdx.y;                        // b * L + l
+  if (g.lay_T) len = __ldg(g.lay_T + bl % g.L) - n_new;   // layer-dependent budgets: this layer's own length
   const bool do_k = what & kAppendK, do_v = what & kAppendV;
   if (do_k && blockIdx.x == 0) {                     // per-update counters of this slab: max of W, pass-1 progress of the tcgen05 scoring
     if (threadIdx.x == 0) g.wmax[bl] = 0u;

@@ -87,7 +87,7 @@ k_gather(Geom g, int cur) {
   const int half = g.d >> 1;
   const int uph = half / V;                                 // units per head
   const int upr = g.Hkv * uph;                              // units per token row
-  const int total = g.budget * upr;
+  const int total = layer_keep(g, bl % g.L) * upr;      // rows this layer holds after the update (its budget, or all of them)
   const size_t slab_src = size_t(bl) * 2 + cur, slab_dst = size_t(bl) * 2 + (cur ^ 1);
   const T* ks = reinterpret_cast<const T*>(g.kc) + slab_src * g.cap * g.row_elems;
   const T* vs = reinterpret_cast<const T*>(g.vc) + slab_src * g.cap * g.row_elems;

@@ -30,7 +30,7 @@ k_score_simt(Geom g, const T* __restrict__ q_probe, int cur, int Tn, int P, floa
   const int kvh = blockIdx.y;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int tok = blockIdx.x * kSimtTokens + tid;
-  const bool valid = tok < Tn;
+  const bool valid = tok < layer_T(g, l, Tn);      // layer-dependent budgets: blocks past T_l contribute (-inf, 0) / nothing
   const int R = g.G * P;                             // probe rows sharing this KV head (contiguous in Q)
   const int row0 = kvh * R;                          // first of them within the layer's Hq*P rows
 

@@ -24,8 +24,9 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_config_struct_matches_header_size():
-    # 15 int32 + 3 float + int32 + 4 float + int32 + float + 3 int32 + 11 int32 = 39 x 4 bytes
-    assert C.sizeof(hb.HermesConfig) == 39 * 4
+    # 15 int32 + 3 float + int32 + 4 float + int32 + float + 3 int32 + 8 int32 + 3 float + 3 int32 = 42 x 4 bytes
+    assert C.sizeof(hb.HermesConfig) == 42 * 4
+    assert list(hb.hermes_default_config().budget_weight) == [1.0, 1.0, 1.0]
     assert hb.hermes_default_config().reindex_mode == 0
     cfg = hb.hermes_default_config()
     assert (cfg.omega0, cfg.gamma) == (0.75, pytest.approx(0.6))
@@ -86,3 +87,14 @@ def test_null_handle_calls_do_not_crash():
     assert lib.hermes_append_chunk(None, None, None, None, 1, 0, -1, None) == hb.HERMES_EINVAL
     assert lib.hermes_len(None) == 0
     lib.hermes_destroy(None)
+
+
+def test_layer_dependent_budget_configs():
+    wl = CONFIGS["llava_ov_7b"]
+    assert hb.hermes_workspace_bytes(hb.config_for_workload(wl, budget_weight=(1.3, 1.0, 0.7))) == 0   # max_tokens < largest layer
+    ok = hb.config_for_workload(wl, budget_weight=(1.3, 1.0, 0.7), max_tokens=0)
+    assert hb.hermes_workspace_bytes(ok) > hb.hermes_workspace_bytes(hb.config_for_workload(wl))   # slabs sized for the largest layer
+    for bad in (dict(budget_weight=(1.3, 1.0, 0.0)), dict(budget_weight=(1.3, 1.0, 0.7), summary_token=1),
+                dict(budget_weight=(1.3, 1.0, 0.7), score_path=hb.HERMES_SCORE_TCGEN05),
+                dict(budget_weight=(0.7, 1.0, 1.3), rope_mode=hb.HERMES_ROPE_M3D)):
+        assert hb.hermes_workspace_bytes(hb.config_for_workload(wl, max_tokens=0, **bad)) == 0

@@ -82,6 +82,9 @@ class _FakeEvent:
     def elapsed_time(self, other):
         return (other.t - self.t) * 1e3
 
+    def synchronize(self):
+        pass
+
 
 class _CpuBackend:
     """Stand-in for bench.CudaBackend: CPU tensors, wall-clock events, gloo."""

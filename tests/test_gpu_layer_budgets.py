@@ -1,0 +1,109 @@
+"""GPU parity for layer-dependent budgets (Tab. 5; DESIGN f4): the CUDA path through the C ABI
+against oracle_step_layer_budgets, lock-step, at the three non-uniform weightings of Tab. 5."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2601_14724_b200 as hb
+from gpu_harness import BAND_RTOL, K_RTOL, SCORE_RTOL, to_dev
+from helpers import Feeder, bf16_ulp, oracle_config
+from oracle import hermes_oracle as ho
+from workloads import CONFIGS
+
+pytestmark = pytest.mark.gpu
+TAB5 = [(1.3, 1.0, 0.7), (0.7, 1.6, 0.7), (0.7, 1.0, 1.3)]
+
+
+def _gpu_state(h, ocfg, wl):
+    """Oracle stream holding the GPU's current cache (per-layer lengths)."""
+    torch.cuda.synchronize()
+    st = ho.OracleStream(ocfg)
+    L = wl.n_layers
+    st.lens = np.array([hb.hermes_layer_len(h, l) for l in range(L)], np.int64)
+    st.len = int(st.lens.max())
+    st._ensure(max(st.len, 1))
+    for l in range(L):
+        v = hb.hermes_get_cache(h, 0, l)
+        n = int(st.lens[l])
+        assert v["len"] == n
+        st.K[l, :n] = v["k"].float().cpu().numpy(); st.V[l, :n] = v["v"].float().cpu().numpy()
+        st.pos[l, :, :n] = v["pos"].cpu().numpy()
+    return st
+
+
+def _run(wl, w, n_updates, **over):
+    ocfg = oracle_config(wl, budget_weights=w, capacity=0)
+    m = ho.layer_budgets(ocfg)
+    # slots per layer: the largest layer plus a chunk, and at least the workload's own capacity (the toy preload)
+    cfg = hb.config_for_workload(wl, budget_weight=w, max_tokens=int(max(wl.cap, m.max() + wl.chunk_tokens)), **over)
+    h = hb.hermes_create(cfg)
+    assert [hb.hermes_layer_budget(h, l) for l in range(wl.n_layers)] == m.tolist()
+    fd = Feeder(wl, 0)
+    half = wl.head_dim // 2
+    n_cmp = n_untouched = 0
+    sizes = [wl.preload_tokens] if wl.preload_tokens else []
+    for u, n in enumerate(sizes + [wl.chunk_tokens] * n_updates):
+        st = _gpu_state(h, ocfg, wl)
+        ap = ho.arrival_positions(ocfg, st, n, -1)
+        K, V, Q, _ = fd.next(n, ap, with_probe=u >= len(sizes))
+        hb.hermes_append_chunk(h, to_dev(K[None], wl.dtype), to_dev(V[None], wl.dtype), None if Q is None else to_dev(Q[None], wl.dtype))
+        torch.cuda.synchronize()
+        out = ho.oracle_step_layer_budgets(st, K, V, Q)
+        assert hb.hermes_len(h) == int(st.lens.max())
+        for l in range(wl.n_layers):
+            v = hb.hermes_get_cache(h, 0, l)
+            n_l = int(st.lens[l])
+            assert v["len"] == n_l == hb.hermes_layer_len(h, l)
+            k_gpu = v["k"].float().cpu().numpy(); v_gpu = v["v"].float().cpu().numpy(); p_gpu = v["pos"].cpu().numpy()
+            if not out["evicted"] or not out["evicted_layers"][l]:          # appended to, otherwise untouched: bit-exact
+                assert np.array_equal(k_gpu, st.K[l, :n_l]) and np.array_equal(v_gpu, st.V[l, :n_l])
+                assert np.array_equal(p_gpu, st.pos[l, :, :n_l])
+                n_untouched += bool(out["evicted"])
+                continue
+            assert v["last_T"] == out["T"][l]
+            s_gpu = v["last_scores"].cpu().numpy().astype(np.float64)
+            s_or = out["S_tilde"][l]
+            rel = np.abs(s_gpu - s_or) / np.maximum(np.abs(s_or), 1e-30)
+            assert (rel <= SCORE_RTOL).all(), f"layer {l}: score rel err {rel.max():.3e}"
+            kept_gpu = v["last_kept"].cpu().numpy().astype(np.int64)
+            kept_or = out["kept"][l]
+            assert len(kept_gpu) == m[l] and (np.diff(kept_gpu) > 0).all()
+            if not np.array_equal(kept_gpu, kept_or):
+                tau = s_or[kept_or].min()
+                diff = np.setxor1d(kept_gpu, kept_or)
+                assert (np.abs(s_or[diff] - tau) <= BAND_RTOL * abs(tau)).all(), f"layer {l}: kept sets differ outside the band"
+                continue
+            assert np.array_equal(p_gpu, st.pos[l, :, :n_l])
+            assert np.array_equal(v_gpu.view(np.uint32), st.V[l, :n_l].view(np.uint32))
+            ko = st.K[l, :n_l]
+            nrm = np.hypot(ko[..., :half].astype(np.float64), ko[..., half:].astype(np.float64))
+            tol = K_RTOL * np.concatenate([nrm, nrm], -1)
+            if wl.dtype == "bf16":
+                tol = np.maximum(tol, 2 * bf16_ulp(ko))
+            assert (np.abs(k_gpu.astype(np.float64) - ko) <= tol + 1e-30).all(), f"layer {l}: K beyond tolerance"
+            n_cmp += 1
+    assert hb.hermes_device_status(h) == 0 and hb.hermes_last_score_path(h) == hb.HERMES_SCORE_SIMT
+    lens = [hb.hermes_layer_len(h, l) for l in range(wl.n_layers)]
+    hb.hermes_destroy(h)
+    return m, lens, n_cmp, n_untouched
+
+
+@pytest.mark.parametrize("w", TAB5)
+def test_toy_config_at_tab5_weightings(w):
+    wl = CONFIGS["toy"]                                       # fp32, 4 layers (1 / 2 / 1), preload 128, chunks of 32
+    m, lens, n_cmp, n_untouched = _run(wl, w, 8)
+    assert lens == m.tolist() and n_cmp >= 20
+    if m.max() > 160:
+        assert n_untouched > 0                                # a big layer was still under its budget while others compressed
+
+
+def test_bf16_geometry_at_tab5_weighting():
+    wl = CONFIGS["llava_ov_7b"].scaled(n_layers=7, budget=588, probe_tokens=8)     # 1 / 4 / 2 layers, bf16, d 128
+    m, lens, n_cmp, _ = _run(wl, (0.7, 1.0, 1.3), 6)
+    assert lens == np.minimum(m, 196 * 6).tolist() and n_cmp >= 14
+
+
+def test_equal_weights_are_the_uniform_path():
+    wl = CONFIGS["toy"]
+    m, lens, n_cmp, n_untouched = _run(wl, (2.0, 2.0, 2.0), 3)
+    assert lens == [wl.budget] * wl.n_layers and n_untouched == 0
