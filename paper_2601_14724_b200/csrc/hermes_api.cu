@@ -94,7 +94,7 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   {
     cudaFuncAttributes fa;
     CUDA_TRY(nullptr, cudaFuncGetAttributes(&fa, k_select));
-    if (fa.sharedSizeBytes + size_t(sel_quarter(y.cap)) * 4 > prop.sharedMemPerBlockOptin)
+    if (fa.sharedSizeBytes + size_t(y.cap) * 4 > prop.sharedMemPerBlockOptin)
       return fail(nullptr, HERMES_EINVAL, "max_tokens %d too large for the select kernel's shared memory", y.cap);
     if (c->summary_token) {
       const size_t need = size_t(y.cap - c->budget + 2) * 8;
@@ -190,7 +190,7 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   if (e == cudaSuccess) e = cudaMemset(g.status, 0, 256);
   if (e == cudaSuccess) e = cudaMemset(h->ws + y.seg_cnt, 0, size_t(g.B) * L * y.n_vh_max * 4);
   if (e == cudaSuccess) e = cudaMemset(g.posc, 0, size_t(g.B) * L * 2 * y.n_axes * y.cap * 4);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_select, cudaFuncAttributeMaxDynamicSharedMemorySize, sel_quarter(y.cap) * 4);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_select, cudaFuncAttributeMaxDynamicSharedMemorySize, y.cap * 4);
   if (e == cudaSuccess) e = cudaDeviceSynchronize();
   if (e != cudaSuccess) {
     fail(nullptr, HERMES_ECUDA, "create: %s", cudaGetErrorString(e));
@@ -448,7 +448,7 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
       const float r_norm_sum = float((1.0 - std::exp(-k)) / (1.0 - std::exp(-k * Tn)));
       if (g.L > g.n_shallow)
         launch_pdl(k_wsum, dim3((Tn + 255) / 256, g.B * (g.L - g.n_shallow)), dim3(256), 0, s, g, Tn, n_probe, h->n_vh);
-      launch_pdl(k_select, dim3(BL * kSelCluster), dim3(kSelThreads), size_t(sel_quarter(Tn)) * 4, s, g, h->cur, Tn, c.forget_rate, int(c.norm_mode == HERMES_NORM_SUM), r_norm_sum, int(reindex),
+      launch_pdl(k_select, dim3(BL), dim3(kSelThreads), size_t(Tn) * 4, s, g, h->cur, Tn, c.forget_rate, int(c.norm_mode == HERMES_NORM_SUM), r_norm_sum, int(reindex),
                  reindex ? c.pos_offset + c.budget - 1 : int(p0 + span));
     }
     if (c.summary_token && h->lay.n_deep > 0) {

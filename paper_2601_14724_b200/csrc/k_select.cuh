@@ -5,19 +5,18 @@
 //       (score, index) -- ties evict the smaller index -- then a flag scan that emits I_l ascending
 //   a6  new positions (Eq. 8: offset + rank; Eq. 11: per-axis rank among DISTINCT retained coordinates)
 // Scores live in shared memory for the whole block; W^l and W^{l+1} are re-read from L2.
-//
-// One thread block CLUSTER of kSelCluster CTAs per (stream, layer): CTA r owns a contiguous quarter of the candidates
-// (a multiple of 32 tokens), every phase runs on the quarter, and the three places where the quarters meet -- the digit
-// histogram of each radix round, the evicted-count prefix of the flag scan, and (M-RoPE) the coordinate bitmap -- are
-// exchanged through distributed shared memory.  Every CTA reaches the same threshold from the same summed histogram.
 #pragma once
-#include <cooperative_groups.h>
 #include "common.cuh"
 
 namespace hk {
 
+#ifdef HERMES_SELECT_TIMING
+#define SEL_T(n) do { __syncthreads(); if (blockIdx.x == 5 && threadIdx.x == 0) tstamp[n] = clock64(); } while (0)
+#else
+#define SEL_T(n)
+#endif
+
 constexpr int kSelThreads = 1024;
-constexpr int kSelCluster = 4;                       // CTAs per (stream, layer)
 constexpr int kBitmapWords = 2048;                   // 65536 coordinate values per axis
 
 __device__ inline uint32_t orderable(float f) {      // monotone float -> uint32 map
@@ -110,13 +109,9 @@ k_wsum(Geom g, int Tn, int P, int n_vh) {
   }
 }
 
-// Candidates per CTA of the cluster: a multiple of 32, so that the 32-token flag chunks never straddle two CTAs.
-__host__ __device__ inline int sel_quarter(int Tn) { return (Tn + kSelCluster * 32 - 1) / (kSelCluster * 32) * 32; }
-
-__global__ void __cluster_dims__(kSelCluster, 1, 1) __launch_bounds__(kSelThreads)
+__global__ void __launch_bounds__(kSelThreads)
 k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum, int reindex, int summary_pos) {
-  namespace cg = cooperative_groups;
-  extern __shared__ float s_sc[];                    // [Tq] smoothed scores of this CTA's candidates
+  extern __shared__ float s_sc[];                    // [Tn] smoothed scores
   // per-warp digit histograms (radix phase); the M-RoPE rank bitmap + word prefixes reuse the space later
   __shared__ __align__(16) int whist[32 * 256];
   __shared__ int part[4][256];
@@ -125,16 +120,16 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
   __shared__ int red_i[32];
   __shared__ uint32_t sel_prefix;
   __shared__ int sel_remaining;
-  __shared__ int xhist[2][256];                      // this CTA's digit histogram of a radix round (by round parity): read by the whole cluster
-  __shared__ int xtot;                               // this CTA's packed (#key < v*, #key == v*): read by the higher ranks
   uint32_t* bitmap = reinterpret_cast<uint32_t*>(whist);              // [kBitmapWords]
   int* word_prefix = whist + kBitmapWords;                            // [kBitmapWords]
 
+#ifdef HERMES_SELECT_TIMING
+  __shared__ long long tstamp[8];
+#endif
   pdl_wait();
   pdl_launch_dependents();
-  cg::cluster_group cluster = cg::this_cluster();
-  const int rank = int(cluster.block_rank());
-  const int bl = blockIdx.x / kSelCluster, l = bl % g.L;
+  SEL_T(0);
+  const int bl = blockIdx.x, l = bl % g.L;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   // layer-dependent budgets (DESIGN f4): this layer's own candidates and budget; Eq. 5 pairs candidate i with candidate
   // i + shift1 of layer l + 1 (equal distance from the newest token), candidates without a counterpart keep S^l
@@ -142,8 +137,6 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
   Tn = layer_T(g, l, Tn);
   const int shift1 = T1 - Tn;
   const int budget_l = layer_keep(g, l);
-  const int Tq = sel_quarter(Tn);
-  const int i_beg = min(Tn, rank * Tq), i_end = min(Tn, i_beg + Tq), n_loc = i_end - i_beg;   // this CTA's candidates
   const bool scored0 = l >= g.n_shallow;
   const bool has_next = l + 1 < g.L;
   const bool scored1 = has_next && (l + 1 >= g.n_shallow);
@@ -152,7 +145,7 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
   const float* w0 = g.wsum + size_t(bl) * g.cap;
   const float* w1 = w0 + g.cap;
   float n0, n1;
-  if (norm_sum) {                                    // every CTA sums the whole layer: same order, same value
+  if (norm_sum) {
     float t0 = 0.f, t1 = 0.f;
     for (int i = tid; i < max(Tn, T1); i += kSelThreads) { if (scored0 && i < Tn) t0 += __ldcg(w0 + i); if (scored1 && i < T1) t1 += __ldcg(w1 + i); }
     n0 = block_reduce_sum(t0, red_f);
@@ -170,20 +163,21 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
     r_norm1 = float((1.0 - exp(-double(k_forget))) / (1.0 - exp(-double(k_forget) * T1)));
   }
 
+  SEL_T(1);
   // ---- a2/a3: S^l, S^{l+1}, S~^l (4 tokens per thread per trip: all loads issued before use) ----
   float* scores_out = g.scores + size_t(bl) * g.cap;
-  for (int j0 = tid; j0 < n_loc; j0 += 4 * kSelThreads) {
+  for (int i0 = tid; i0 < Tn; i0 += 4 * kSelThreads) {
     float x0[4], x1[4];
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
-      const int i = i_beg + j0 + j * kSelThreads;
-      x0[j] = (scored0 && i < i_end) ? __ldcg(w0 + i) : 0.f;
-      x1[j] = (scored1 && i < i_end && i + shift1 >= 0) ? __ldcg(w1 + i + shift1) : 0.f;
+      const int i = i0 + j * kSelThreads;
+      x0[j] = (scored0 && i < Tn) ? __ldcg(w0 + i) : 0.f;
+      x1[j] = (scored1 && i < Tn && i + shift1 >= 0) ? __ldcg(w1 + i + shift1) : 0.f;
     }
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
-      const int i = i_beg + j0 + j * kSelThreads;
-      if (i < i_end) {
+      const int i = i0 + j * kSelThreads;
+      if (i < Tn) {
         const float e = expf(-k_forget * float(Tn - 1 - i));                 // Eq. 1
         const float R = e * r_norm;
         float sc = (1.0f - om0) * (x0[j] * a0) + om0 * R;                    // Eq. 2, Eq. 4
@@ -191,7 +185,7 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
           const float s1 = (1.0f - om1) * (x1[j] * a1) + om1 * (e * r_norm1);
           sc = (1.0f - lam) * sc + lam * s1;                                 // Eq. 5
         }
-        s_sc[i - i_beg] = sc;
+        s_sc[i] = sc;
         scores_out[i] = sc;
       }
     }
@@ -199,31 +193,34 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
   // deep layers of a summary-token cache keep one token fewer: slot budget-1 is the summary token (DESIGN f1)
   const bool summ = g.summary && l >= g.L - g.n_deep;
   const int n_keep = budget_l - (summ ? 1 : 0);
-  int32_t* kept = g.kept + size_t(bl) * g.budget;
-  const int32_t* pos_old = g.posc + (size_t(bl) * 2 + cur) * g.n_axes * g.cap;
-  int32_t* pos_new = g.posc + (size_t(bl) * 2 + (cur ^ 1)) * g.n_axes * g.cap;
-  int32_t* dl1 = g.delta + size_t(bl) * g.n_axes * g.budget;
   if (n_keep >= Tn) {
     // layer-dependent budgets: this layer is under its budget at this arrival -- nothing is evicted, nothing re-indexed
     // (1D RoPE only, validated at create); the gather then copies every row as it is
-    for (int i = i_beg + tid; i < i_end; i += kSelThreads) { kept[i] = i; dl1[i] = 0; pos_new[i] = __ldcg(pos_old + i); }
-    return;                                          // the whole cluster takes this branch: no barrier is left waiting
+    const int32_t* po = g.posc + (size_t(bl) * 2 + cur) * g.n_axes * g.cap;
+    int32_t* pn = g.posc + (size_t(bl) * 2 + (cur ^ 1)) * g.n_axes * g.cap;
+    for (int i = tid; i < Tn; i += kSelThreads) {
+      g.kept[size_t(bl) * g.budget + i] = i;
+      g.delta[size_t(bl) * g.n_axes * g.budget + i] = 0;
+      pn[i] = __ldcg(po + i);
+    }
+    return;
   }
   if (tid == 0) { sel_prefix = 0u; sel_remaining = Tn - n_keep; }
   for (int i = tid; i < 32 * 256; i += kSelThreads) whist[i] = 0;
   __syncthreads();
 
+  SEL_T(2);
   // ---- a4: radix select of the E-th smallest key (8 bits per round, MSB first) ------------------
   for (int round = 0; round < 4; ++round) {
     const int shift = 24 - 8 * round;
     const uint32_t himask = round == 0 ? 0u : (0xFFFFFFFFu << (shift + 8));
     const uint32_t prefix = sel_prefix;
     int* my_hist = whist + warp * 256;
-    for (int j0 = 0; j0 < n_loc; j0 += kSelThreads) {    // whole warps iterate together
-      const int j = j0 + tid;
+    for (int i0 = 0; i0 < Tn; i0 += kSelThreads) {     // whole warps iterate together
+      const int i = i0 + tid;
       uint32_t digit = 0xFFFFFFFFu;
-      if (j < n_loc) {
-        const uint32_t key = orderable(s_sc[j]);
+      if (i < Tn) {
+        const uint32_t key = orderable(s_sc[i]);
         if ((key & himask) == prefix) digit = (key >> shift) & 255u;
       }
       // warp-private histogram: the shared-memory atomics only ever collide inside one warp
@@ -238,19 +235,14 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
       part[q][d] = c;
     }
     __syncthreads();
-    if (tid < 256) xhist[round & 1][tid] = (part[0][tid] + part[1][tid]) + (part[2][tid] + part[3][tid]);
-    cluster.sync();                                     // every CTA's histogram of this round is in its shared memory
-    if (warp == 0) {                                    // find the bucket holding the E-th smallest (same result in every CTA)
+    if (warp == 0) {                                    // find the bucket holding the E-th smallest
       int c[8], tot = 0;
 #pragma unroll
-      for (int j = 0; j < 8; ++j) c[j] = 0;
-      for (int r = 0; r < kSelCluster; ++r) {
-        const int* xh = cluster.map_shared_rank(&xhist[round & 1][0], r);
-#pragma unroll
-        for (int j = 0; j < 8; ++j) c[j] += xh[lane * 8 + j];
+      for (int j = 0; j < 8; ++j) {
+        const int d = lane * 8 + j;
+        c[j] = (part[0][d] + part[1][d]) + (part[2][d] + part[3][d]);
+        tot += c[j];
       }
-#pragma unroll
-      for (int j = 0; j < 8; ++j) tot += c[j];
       int inc = tot;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) {
@@ -273,60 +265,61 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
     }
     __syncthreads();
   }
+  SEL_T(3);
   const uint32_t vstar = sel_prefix;                    // key of the E-th smallest score
   const int r_eq = sel_remaining;                       // evicted among keys == vstar (smallest indices)
 
   // ---- flags + one packed scan over 32-token chunks; outputs are written coalesced -------------
   // evicted(i) = key < v*  or  (key == v* and fewer than r_eq equal keys precede i)
-  // chunk c = this CTA's tokens [32c, 32c+32): cnt_c = #(key < v*) | #(key == v*) << 16, exclusive-scanned over c.
-  const int n_chunks = (n_loc + 31) >> 5;
+  // chunk c = tokens [32c, 32c+32): cnt_c = #(key < v*) | #(key == v*) << 16, exclusive-scanned over c.
+  const int n_chunks = (Tn + 31) >> 5;                                   // <= 1024 * kChunkPerThread
   int* chunk_pre = whist;                                                // reuse: [n_chunks] packed prefixes
+  SEL_T(4);
   for (int c = warp; c < n_chunks; c += 32) {
-    const int j = c * 32 + lane;
-    const uint32_t key = j < n_loc ? orderable(s_sc[j]) : 0xFFFFFFFFu;
-    const uint32_t lt = __ballot_sync(0xffffffffu, j < n_loc && key < vstar);
-    const uint32_t eq = __ballot_sync(0xffffffffu, j < n_loc && key == vstar);
+    const int i = c * 32 + lane;
+    const uint32_t key = i < Tn ? orderable(s_sc[i]) : 0xFFFFFFFFu;
+    const uint32_t lt = __ballot_sync(0xffffffffu, i < Tn && key < vstar);
+    const uint32_t eq = __ballot_sync(0xffffffffu, i < Tn && key == vstar);
     if (lane == 0) chunk_pre[c] = __popc(lt) | (__popc(eq) << 16);
   }
   __syncthreads();
   {
-    const int cpt = (n_chunks + kSelThreads - 1) / kSelThreads;          // chunks per thread (1 up to 128K candidates)
+    const int cpt = (n_chunks + kSelThreads - 1) / kSelThreads;          // chunks per thread (1 up to 32K tokens)
     const int c_beg = min(tid * cpt, n_chunks), c_end = min(c_beg + cpt, n_chunks);
     int mine = 0;
     for (int c = c_beg; c < c_end; ++c) mine += chunk_pre[c];
     int tot;
     int run = block_exscan(mine, warp_tot, &tot);                        // both halves stay < 65536
     for (int c = c_beg; c < c_end; ++c) { const int v = chunk_pre[c]; chunk_pre[c] = run; run += v; }
-    if (tid == 0) xtot = tot;
   }
-  cluster.sync();                                                        // totals of the lower ranks (and chunk_pre) are in place
-  int lt_off = 0, eq_off = 0;
-  for (int r = 0; r < rank; ++r) {
-    const int t = *cluster.map_shared_rank(&xtot, r);
-    lt_off += t & 0xFFFF; eq_off += t >> 16;
-  }
+  __syncthreads();
+  SEL_T(6);
+  int32_t* kept = g.kept + size_t(bl) * g.budget;
+  const int32_t* pos_old = g.posc + (size_t(bl) * 2 + cur) * g.n_axes * g.cap;
+  int32_t* pos_new = g.posc + (size_t(bl) * 2 + (cur ^ 1)) * g.n_axes * g.cap;
+  int32_t* dl1 = g.delta + size_t(bl) * g.n_axes * g.budget;
   const uint32_t lane_lt = (1u << lane) - 1u;
   for (int cb = warp; cb < n_chunks; cb += 32 * 8) {                     // 8 chunks per trip: old positions first
     int p_old[8];
 #pragma unroll
     for (int j = 0; j < 8; ++j) {
-      const int i = i_beg + (cb + 32 * j) * 32 + lane;
-      p_old[j] = (g.n_axes == 1 && i < i_end) ? __ldcg(pos_old + i) : 0;
+      const int i = (cb + 32 * j) * 32 + lane;
+      p_old[j] = (g.n_axes == 1 && i < Tn) ? __ldcg(pos_old + i) : 0;
     }
 #pragma unroll
     for (int j = 0; j < 8; ++j) {
       const int c = cb + 32 * j;                                         // warp-uniform
       if (c >= n_chunks) break;
-      const int jl = c * 32 + lane, i = i_beg + jl;
-      const uint32_t key = jl < n_loc ? orderable(s_sc[jl]) : 0xFFFFFFFFu;
-      const uint32_t lt = __ballot_sync(0xffffffffu, jl < n_loc && key < vstar);
-      const uint32_t eq = __ballot_sync(0xffffffffu, jl < n_loc && key == vstar);
+      const int i = c * 32 + lane;
+      const uint32_t key = i < Tn ? orderable(s_sc[i]) : 0xFFFFFFFFu;
+      const uint32_t lt = __ballot_sync(0xffffffffu, i < Tn && key < vstar);
+      const uint32_t eq = __ballot_sync(0xffffffffu, i < Tn && key == vstar);
       const int pre = chunk_pre[c];
-      const int lt_before = lt_off + (pre & 0xFFFF) + __popc(lt & lane_lt);
-      const int eq_before = eq_off + (pre >> 16) + __popc(eq & lane_lt);
+      const int lt_before = (pre & 0xFFFF) + __popc(lt & lane_lt);
+      const int eq_before = (pre >> 16) + __popc(eq & lane_lt);
       const bool evict = key < vstar || (key == vstar && eq_before < r_eq);
-      if (summ && jl < n_loc && evict) g.evicted[size_t(bl) * g.n_evict_max + lt_before + min(eq_before, r_eq)] = i;
-      if (jl < n_loc && !evict) {
+      if (summ && i < Tn && evict) g.evicted[size_t(bl) * g.n_evict_max + lt_before + min(eq_before, r_eq)] = i;
+      if (i < Tn && !evict) {
         const int out = i - lt_before - min(eq_before, r_eq);            // slot of token i among the kept
         kept[out] = i;
         if (g.n_axes == 1) {                                             // Eq. 8: positions rise with the index -> rank = slot
@@ -337,40 +330,42 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
       }
     }
   }
-  if (summ && rank == 0 && tid == 0) {                  // the summary token's slot (filled by k_summary)
+#ifdef HERMES_SELECT_TIMING
+  SEL_T(5);
+  if (blockIdx.x == 5 && threadIdx.x == 0) printf("select phases (cycles): setup %lld scores %lld radix %lld count+scan %lld write %lld\n", tstamp[1]-tstamp[0], tstamp[2]-tstamp[1], tstamp[3]-tstamp[2], tstamp[6]-tstamp[4], tstamp[5]-tstamp[6]);
+#endif
+  if (summ && tid == 0) {                               // the summary token's slot (filled by k_summary)
     kept[n_keep] = -1; pos_new[n_keep] = summary_pos; dl1[n_keep] = 0;
   }
-  // no CTA may exit while another one can still read its shared memory (xtot above)
-  __threadfence();
-  cluster.sync();
-  if (g.n_axes == 1 || rank != 0) return;
+  if (g.n_axes == 1) return;
+  __syncthreads();                                      // kept[] visible to the whole block
 
-  // ---- a6 (M-RoPE): per-axis rank among the distinct retained coordinates (Eq. 11); CTA 0 of the cluster ---------
+  // ---- a6 (M-RoPE): per-axis rank among the distinct retained coordinates (Eq. 11) ----------------
   for (int a = 0; a < 3; ++a) {
     const int32_t* po = pos_old + size_t(a) * g.cap;
     int32_t* pn = pos_new + size_t(a) * g.cap;
     int32_t* dl = g.delta + (size_t(bl) * 3 + a) * g.budget;
     if (!reindex || !((g.compact_axes >> a) & 1)) {     // axis kept as is (DESIGN c13; lazy mode between re-index steps)
-      for (int s = tid; s < g.budget; s += kSelThreads) { pn[s] = __ldcg(po + __ldcg(kept + s)); dl[s] = 0; }
+      for (int s = tid; s < g.budget; s += kSelThreads) { pn[s] = __ldcg(po + kept[s]); dl[s] = 0; }
       continue;
     }
     int vmin = INT_MAX, vmax_neg = INT_MAX;
     for (int s = tid; s < g.budget; s += kSelThreads) {
-      const int v = __ldcg(po + __ldcg(kept + s));
+      const int v = __ldcg(po + kept[s]);
       vmin = min(vmin, v); vmax_neg = min(vmax_neg, -v);
     }
     vmin = block_reduce_min_i(vmin, red_i);
     const int vmax = -block_reduce_min_i(vmax_neg, red_i);
     if (vmax - vmin >= kBitmapWords * 32) {             // cannot rank: report, leave the axis untouched
       if (tid == 0) atomicOr(g.status, 1);
-      for (int s = tid; s < g.budget; s += kSelThreads) { pn[s] = __ldcg(po + __ldcg(kept + s)); dl[s] = 0; }
+      for (int s = tid; s < g.budget; s += kSelThreads) { pn[s] = __ldcg(po + kept[s]); dl[s] = 0; }
       continue;
     }
     __syncthreads();
     for (int w = tid; w < kBitmapWords; w += kSelThreads) bitmap[w] = 0u;
     __syncthreads();
     for (int s = tid; s < g.budget; s += kSelThreads) {
-      const int v = __ldcg(po + __ldcg(kept + s)) - vmin;
+      const int v = __ldcg(po + kept[s]) - vmin;
       atomicOr(&bitmap[v >> 5], 1u << (v & 31));
     }
     __syncthreads();
@@ -381,7 +376,7 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
     word_prefix[2 * tid + 1] = wpre + __popc(bitmap[2 * tid]);
     __syncthreads();
     for (int s = tid; s < g.budget; s += kSelThreads) {
-      const int v = __ldcg(po + __ldcg(kept + s)) - vmin;
+      const int v = __ldcg(po + kept[s]) - vmin;
       const int p_new = g.pos_offset + word_prefix[v >> 5] + __popc(bitmap[v >> 5] & ((1u << (v & 31)) - 1u));
       pn[s] = p_new;
       dl[s] = p_new - (v + vmin);
