@@ -127,6 +127,10 @@ void hermes_default_config(hermes_config *cfg);
 /* Bytes of device workspace a handle with this config needs; 0 if the config is invalid.              */
 size_t hermes_workspace_bytes(const hermes_config *cfg);
 
+/* Per-layer budgets m_i of a config (hermes_config.budget_weight): writes min(n, n_layers) values to out
+ * and returns n_layers, or HERMES_EINVAL for an invalid config.  Host-only: needs no device.                         */
+int hermes_layer_budgets(const hermes_config *cfg, int32_t *out, int32_t n);
+
 /* Validates cfg (HERMES_EINVAL: H_q % H_kv != 0, head_dim not in {32,64,128}, sum(mrope_section) !=
  * head_dim/2, budget <= 0, forget_rate <= 0, n_shallow + n_deep > L, ...), binds `workspace`
  * (device pointer, `bytes` >= hermes_workspace_bytes, else HERMES_ECAPACITY), builds the rotary table

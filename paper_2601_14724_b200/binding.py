@@ -21,7 +21,7 @@ HERMES_SCORE_AUTO, HERMES_SCORE_SIMT, HERMES_SCORE_TCGEN05 = 0, 1, 2
 HERMES_K_NAMES = ("append", "score_stats", "score_combine", "score_colsum", "select", "gather", "summary")
 
 EXPORTS = ("hermes_default_config", "hermes_workspace_bytes", "hermes_create", "hermes_append_chunk",
-           "hermes_append_chunk_host", "hermes_get_cache", "hermes_len", "hermes_layer_len", "hermes_layer_budget", "hermes_device_status",
+           "hermes_append_chunk_host", "hermes_get_cache", "hermes_len", "hermes_layer_len", "hermes_layer_budget", "hermes_layer_budgets", "hermes_device_status",
            "hermes_set_profiling", "hermes_get_profile", "hermes_last_score_path", "hermes_v_pending",
            "hermes_last_launch_count", "hermes_destroy", "hermes_last_error")
 
@@ -79,6 +79,7 @@ def load_library(rebuild_if_stale: bool = True) -> C.CDLL:
     lib.hermes_len.argtypes = [vp]
     lib.hermes_layer_len.argtypes = [vp, i32]
     lib.hermes_layer_budget.argtypes = [vp, i32]
+    lib.hermes_layer_budgets.argtypes = [C.POINTER(HermesConfig), C.POINTER(i32), i32]
     lib.hermes_device_status.argtypes = [vp, C.POINTER(i32)]
     lib.hermes_set_profiling.argtypes = [vp, i32]
     lib.hermes_get_profile.argtypes = [vp, C.POINTER(C.c_float), i32]
@@ -107,6 +108,15 @@ def hermes_default_config(**kw) -> HermesConfig:
         else:
             setattr(cfg, k, v)
     return cfg
+
+
+def hermes_layer_budgets(cfg: HermesConfig) -> list:
+    """Per-layer budgets of a config (host-only; no device needed)."""
+    out = (C.c_int32 * max(int(cfg.n_layers), 1))()
+    n = load_library().hermes_layer_budgets(C.byref(cfg), out, len(out))
+    if n < 0:
+        raise HermesError(n, (load_library().hermes_last_error(None) or b"").decode())
+    return list(out[:n])
 
 
 def hermes_workspace_bytes(cfg: HermesConfig) -> int:

@@ -59,6 +59,16 @@ extern "C" size_t hermes_workspace_bytes(const hermes_config* c) {
   return make_layout(*c).total;
 }
 
+extern "C" int hermes_layer_budgets(const hermes_config* c, int32_t* out, int32_t n) {
+  if (!c || !out || n < 0) return HERMES_EINVAL;
+  if (const char* why = validate(*c)) { g_create_error = why; return HERMES_EINVAL; }
+  int ns = c->n_shallow, nd = c->n_deep;
+  stage_split(c->n_layers, ns, nd);
+  const std::vector<int> m = layer_budgets(*c, ns, nd);
+  for (int l = 0; l < c->n_layers && l < n; ++l) out[l] = m[l];
+  return c->n_layers;
+}
+
 extern "C" const char* hermes_last_error(const hermes_t* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 extern "C" int32_t hermes_len(const hermes_t* h) { return h ? h->len : 0; }
 extern "C" int32_t hermes_layer_len(const hermes_t* h, int32_t layer) {

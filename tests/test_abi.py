@@ -98,3 +98,15 @@ def test_layer_dependent_budget_configs():
                 dict(budget_weight=(1.3, 1.0, 0.7), score_path=hb.HERMES_SCORE_TCGEN05),
                 dict(budget_weight=(0.7, 1.0, 1.3), rope_mode=hb.HERMES_ROPE_M3D)):
         assert hb.hermes_workspace_bytes(hb.config_for_workload(wl, max_tokens=0, **bad)) == 0
+
+
+@pytest.mark.parametrize("w", [(1.0, 1.0, 1.0), (1.3, 1.0, 0.7), (0.7, 1.6, 0.7), (0.7, 1.0, 1.3), (0.31, 2.7, 1.9)])
+@pytest.mark.parametrize("L,budget", [(4, 96), (28, 6000), (28, 6272), (80, 4096), (7, 785), (33, 1001)])
+def test_host_layer_budgets_equal_the_oracle(L, budget, w):
+    """The library's host-side allocation against oracle.layer_budgets for the Tab. 5 weightings and an
+    awkward one: same fp32 weights, same fp64 quotient, same residue rule on both sides."""
+    from oracle import hermes_oracle as ho
+    wl = CONFIGS["llava_ov_7b"].scaled(n_layers=L, budget=budget)
+    got = hb.hermes_layer_budgets(hb.config_for_workload(wl, budget_weight=w, max_tokens=0))
+    ocfg = ho.OracleConfig(n_layers=L, n_q_heads=28, n_kv_heads=4, head_dim=128, budget=budget, forget_rate=0.1, budget_weights=w)
+    assert got == ho.layer_budgets(ocfg).tolist() and sum(got) == budget * L
