@@ -27,9 +27,9 @@ from workloads import CONFIGS, chunk_kv, probe_q, sweep_point  # noqa: E402
 METRIC, UNIT = "kv_tokens_managed_per_s", "tokens/s"
 POOL = 16          # distinct pre-generated chunk/probe sets cycled through the timed region
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at configs[1], transcribed from the one
-# `ncu --set full` capture summarised in profiles/r1e_ncu_full_summary.txt (command in profiles/r1e_README.md);
+# `ncu --set full` capture summarised in profiles/r2_ncu_full_summary.txt (command in profiles/r2_README.md);
 # the scoring kernel's figure includes the previous update's V compaction (360 MB) that rides in it
-NCU_TRAFFIC_BYTES = {"gather": 181.35e6 + 132.28e6, "score": 561.65e6 + 192.94e6,
+NCU_TRAFFIC_BYTES = {"gather": 181.35e6 + 132.91e6, "score": 561.52e6 + 189.66e6,
                      "select": 1.44e6, "append": 11.25e6}
 
 
