@@ -26,9 +26,10 @@
  *   - Query head h uses KV head h / (n_q_heads / n_kv_heads) (grouped-query attention).
  *   - A handle is not thread-safe; use one per host thread or serialise calls.
  *   - The tcgen05 scoring kernel is persistent (at most one CTA per SM) and a CTA's second pass waits for row
- *     statistics written by other CTAs of the same launch, so it needs every CTA of its grid resident at once:
- *     run it on a device (or an MPS / green-context partition) whose SMs are not shared with other work while an
- *     update is in flight.
+ *     statistics written by other CTAs of the same launch, so every CTA of its grid must be resident at once.  It is
+ *     launched cooperatively: on a device partition that cannot hold the grid (MPS active-thread percentage, a green
+ *     context) the runtime refuses the launch, and the handle scores on the CUDA-core path from then on
+ *     (HERMES_ECUDA if score_path forces tcgen05).
  */
 #ifndef HERMES_H_
 #define HERMES_H_

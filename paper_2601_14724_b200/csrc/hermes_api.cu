@@ -439,11 +439,24 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
     const float scale = c.softmax_scale > 0.f ? c.softmax_scale : float(1.0 / std::sqrt(double(c.head_dim)));
     const float scale_log2 = scale * kLog2e;
     if (g.L > g.n_shallow) {
+      bool scored = false;
       if (use_tc) {
-        if (int rc = tc_score(h, Q_probe, Tn, n_probe, scale_log2, s, ride && h->v_pending)) return rc;
-        h->v_pending = false;
-        h->last_score_path = HERMES_SCORE_TCGEN05;
-      } else {
+        const int rc = tc_score(h, Q_probe, Tn, n_probe, scale_log2, s, ride && h->v_pending);
+        if (rc == kTcNotResident) {
+          // the device cannot hold one scoring CTA per unit of its grid at once (MPS / green-context partition): this
+          // handle scores on the CUDA-core path from now on; a pending V compaction runs on its own
+          if (c.score_path == HERMES_SCORE_TCGEN05) return fail(h, HERMES_ECUDA, "tcgen05 scoring kernel cannot be made resident on this device partition");
+          h->tc_ok = false;
+          flush_v(h, s);
+        } else if (rc != HERMES_OK) {
+          return rc;
+        } else {
+          h->v_pending = false;
+          h->last_score_path = HERMES_SCORE_TCGEN05;
+          scored = true;
+        }
+      }
+      if (!scored) {
         if (c.dtype == HERMES_BF16) launch_simt<__nv_bfloat16>(h, Q_probe, Tn, n_probe, scale_log2, s);
         else launch_simt<float>(h, Q_probe, Tn, n_probe, scale_log2, s);
         h->last_score_path = HERMES_SCORE_SIMT;

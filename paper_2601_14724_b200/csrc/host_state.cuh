@@ -186,6 +186,21 @@ inline cudaError_t launch_pdl(void (*kernel)(P...), dim3 grid, dim3 block, size_
   return cudaLaunchKernelEx(&cfg, kernel, P(args)...);
 }
 
+// Same, as a COOPERATIVE launch: the runtime refuses the launch (cudaErrorCooperativeLaunchTooLarge) unless every CTA of the
+// grid can be resident at once -- which is what a kernel whose CTAs wait on one another needs.
+template <typename... P, typename... A>
+inline cudaError_t launch_pdl_coop(void (*kernel)(P...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, A... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cudaLaunchAttribute at[2];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  at[1].id = cudaLaunchAttributeCooperative;
+  at[1].val.cooperative = 1;
+  cfg.attrs = at; cfg.numAttrs = 2;
+  return cudaLaunchKernelEx(&cfg, kernel, P(args)...);
+}
+
 struct KernelTimer {
   cudaEvent_t beg[HERMES_K_COUNT]{}, end[HERMES_K_COUNT]{};
   bool ran[HERMES_K_COUNT]{};

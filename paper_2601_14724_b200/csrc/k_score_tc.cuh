@@ -551,9 +551,8 @@ __device__ inline void tc_v_mover(const TcSmem& s, const TcBars& b, const TcArgs
 // One persistent kernel runs both passes: every CTA works through its pass-1 range, then its pass-2
 // range of the same flattened (group, token) space, keeping TMEM, barriers and the K ring alive.  Pass 2
 // of a group only waits (on seg_cnt) for the pass-1 segments of that group, i.e. for this CTA and its
-// schedule neighbours -- there is no grid-wide barrier.  Requires gridDim.x <= #SMs with every CTA resident
-// (an exclusive device: under MPS or an SM-limited context a spinning CTA could starve the one it waits for;
-// include/hermes.h states this).
+// schedule neighbours -- there is no grid-wide barrier.  Requires every CTA resident: the launch is cooperative
+// (gridDim.x <= #SMs; the runtime refuses it on an SM-limited context, and the caller falls back to the CUDA-core path).
 // =====================================================================================================
 __global__ void __launch_bounds__(kTcThreads, 1)
 k_tc_score(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k, TcArgs a) {
@@ -667,6 +666,8 @@ inline bool tc_v_ride_ok(const hermes_t* h, int Tn, int P) {
   return score_us >= 1.25 * (rows_per_cta / per * 3.0);
 }
 
+constexpr int kTcNotResident = 1;   // tc_score: the cooperative launch was refused; the caller scores on the CUDA-core path
+
 struct TcProf {   // same event bracketing as hermes_api.cu's Prof, local to this header
   hermes_t* h; int id; cudaStream_t s;
   TcProf(hermes_t* h_, int id_, cudaStream_t s_) : h(h_), id(id_), s(s_) {
@@ -708,7 +709,12 @@ inline int tc_score(hermes_t* h, const void* q_probe, int Tn, int P, float scale
   const int smem = tc_smem_bytes(a.q_half_bytes, a.n_kst, move_v);
   {
     TcProf p(h, HERMES_K_SCORE_STATS, s);
-    const cudaError_t e = launch_pdl(k_tc_score, dim3(n_cta), dim3(kTcThreads), size_t(smem), s, tmap_q, st->tmap_k, a);
+    // cooperative: pass 2 of a CTA waits for pass-1 statistics of other CTAs, so all of them must be resident
+    const cudaError_t e = launch_pdl_coop(k_tc_score, dim3(n_cta), dim3(kTcThreads), size_t(smem), s, tmap_q, st->tmap_k, a);
+    if (e == cudaErrorCooperativeLaunchTooLarge) {             // not every CTA can be resident (SM-limited context): no spin-waits then
+      (void)cudaGetLastError();
+      return kTcNotResident;
+    }
     if (e != cudaSuccess) { h->err = std::string("tcgen05 scoring launch: ") + cudaGetErrorString(e); return HERMES_ECUDA; }
   }
   return HERMES_OK;
