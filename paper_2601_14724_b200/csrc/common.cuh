@@ -116,27 +116,6 @@ __device__ __forceinline__ float fast_exp2(float x) {
   return y;
 }
 
-// 2^x on the FMA / ALU pipes (no MUFU): round-to-nearest split x = n + f, f in [-0.5, 0.5], degree-4 minimax
-// polynomial for 2^f (max rel. error 2.7e-6, mean 4e-8), exponent patched in with one integer multiply-add.
-// x is clamped at -125, so very negative inputs return ~2^-125 instead of 0 (far below fp32 sum resolution).
-__device__ __forceinline__ float exp2_poly(float x) {
-  const float xc = fmaxf(x, -125.0f);
-  const float r = __fadd_rn(xc, 12582912.0f);                 // 1.5 * 2^23: low mantissa bits = round(xc)
-  const float f = __fsub_rn(xc, __fsub_rn(r, 12582912.0f));
-  float p = 0.009570036083459854f;
-  p = fmaf(p, f, 0.05591771379113197f);
-  p = fmaf(p, f, 0.240247443318367f);
-  p = fmaf(p, f, 0.6931218504905701f);
-  p = fmaf(p, f, 0.9999992847442627f);
-  return __int_as_float(__float_as_int(r) * 0x800000 + __float_as_int(p));   // (round(xc) << 23) + bits(p)
-}
-// exp2 of element j: `kPoly` of every 8 consecutive elements go to the polynomial, the rest to MUFU.EX2,
-// so both pipes work on the same stream of elements.
-template <int kPoly>
-__device__ __forceinline__ float exp2_mix(float x, int j) {
-  return ((j & 7) * kPoly) % 8 < kPoly && kPoly > 0 ? exp2_poly(x) : fast_exp2(x);
-}
-
 // Programmatic dependent launch: every kernel of an update is launched with the programmatic-stream-
 // serialization attribute, so its CTAs may become resident (and run their prologue) while the previous
 // kernel drains.  pdl_wait() blocks until the previous kernel has completed and its writes are visible;

@@ -10,12 +10,6 @@
 
 namespace hk {
 
-#ifdef HERMES_SELECT_TIMING
-#define SEL_T(n) do { __syncthreads(); if (blockIdx.x == 5 && threadIdx.x == 0) tstamp[n] = clock64(); } while (0)
-#else
-#define SEL_T(n)
-#endif
-
 constexpr int kSelThreads = 1024;
 constexpr int kBitmapWords = 2048;                   // 65536 coordinate values per axis
 
@@ -123,12 +117,8 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
   uint32_t* bitmap = reinterpret_cast<uint32_t*>(whist);              // [kBitmapWords]
   int* word_prefix = whist + kBitmapWords;                            // [kBitmapWords]
 
-#ifdef HERMES_SELECT_TIMING
-  __shared__ long long tstamp[8];
-#endif
   pdl_wait();
   pdl_launch_dependents();
-  SEL_T(0);
   const int bl = blockIdx.x, l = bl % g.L;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   // layer-dependent budgets (DESIGN f4): this layer's own candidates and budget; Eq. 5 pairs candidate i with candidate
@@ -162,8 +152,6 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
     r_norm = float((1.0 - exp(-double(k_forget))) / (1.0 - exp(-double(k_forget) * Tn)));
     r_norm1 = float((1.0 - exp(-double(k_forget))) / (1.0 - exp(-double(k_forget) * T1)));
   }
-
-  SEL_T(1);
   // ---- a2/a3: S^l, S^{l+1}, S~^l (4 tokens per thread per trip: all loads issued before use) ----
   float* scores_out = g.scores + size_t(bl) * g.cap;
   for (int i0 = tid; i0 < Tn; i0 += 4 * kSelThreads) {
@@ -208,8 +196,6 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
   if (tid == 0) { sel_prefix = 0u; sel_remaining = Tn - n_keep; }
   for (int i = tid; i < 32 * 256; i += kSelThreads) whist[i] = 0;
   __syncthreads();
-
-  SEL_T(2);
   // ---- a4: radix select of the E-th smallest key (8 bits per round, MSB first) ------------------
   for (int round = 0; round < 4; ++round) {
     const int shift = 24 - 8 * round;
@@ -265,7 +251,6 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
     }
     __syncthreads();
   }
-  SEL_T(3);
   const uint32_t vstar = sel_prefix;                    // key of the E-th smallest score
   const int r_eq = sel_remaining;                       // evicted among keys == vstar (smallest indices)
 
@@ -274,7 +259,6 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
   // chunk c = tokens [32c, 32c+32): cnt_c = #(key < v*) | #(key == v*) << 16, exclusive-scanned over c.
   const int n_chunks = (Tn + 31) >> 5;                                   // <= 1024 * kChunkPerThread
   int* chunk_pre = whist;                                                // reuse: [n_chunks] packed prefixes
-  SEL_T(4);
   for (int c = warp; c < n_chunks; c += 32) {
     const int i = c * 32 + lane;
     const uint32_t key = i < Tn ? orderable(s_sc[i]) : 0xFFFFFFFFu;
@@ -293,7 +277,6 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
     for (int c = c_beg; c < c_end; ++c) { const int v = chunk_pre[c]; chunk_pre[c] = run; run += v; }
   }
   __syncthreads();
-  SEL_T(6);
   int32_t* kept = g.kept + size_t(bl) * g.budget;
   const int32_t* pos_old = g.posc + (size_t(bl) * 2 + cur) * g.n_axes * g.cap;
   int32_t* pos_new = g.posc + (size_t(bl) * 2 + (cur ^ 1)) * g.n_axes * g.cap;
@@ -330,10 +313,6 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
       }
     }
   }
-#ifdef HERMES_SELECT_TIMING
-  SEL_T(5);
-  if (blockIdx.x == 5 && threadIdx.x == 0) printf("select phases (cycles): setup %lld scores %lld radix %lld count+scan %lld write %lld\n", tstamp[1]-tstamp[0], tstamp[2]-tstamp[1], tstamp[3]-tstamp[2], tstamp[6]-tstamp[4], tstamp[5]-tstamp[6]);
-#endif
   if (summ && tid == 0) {                               // the summary token's slot (filled by k_summary)
     kept[n_keep] = -1; pos_new[n_keep] = summary_pos; dl1[n_keep] = 0;
   }
