@@ -33,7 +33,8 @@ constexpr int kTcRegsLaunch = 96;                // registers per thread at laun
 constexpr int kTcRegsCtl = 64, kTcRegsEpi = 104; // setmaxnreg: warpgroup 0 releases registers, the epilogue warps take them
 // setmaxnreg.inc draws only on registers released by setmaxnreg.dec in the same CTA -- it spins forever otherwise
 static_assert((kTcRegsLaunch - kTcRegsCtl) * kTcCtlWarps >= (kTcRegsEpi - kTcRegsLaunch) * kTcEpiWarps, "register pool");
-constexpr int kTcMoverRing = 32768;             // shared-memory staging of the V mover
+constexpr int kTcMoverRingMax = 32768;          // shared-memory staging of the V mover: at most 32 KB ...
+constexpr int kTcMoverRowsMin = 8;              // ... and at least 8 rows per batch, else the move does not ride
 constexpr int kTcSegTiles = 4;                  // pass 1: 128-token tiles per segment (one partial pair per
                                                 // segment, so the merge order never depends on the CTA schedule)
 
@@ -51,6 +52,7 @@ struct TcArgs {
   const char* v_base;       // V cache base, or NULL: nothing pending
   const int32_t* v_kept;    // [B*L][budget] kept lists of the previous update
   int v_src_buf, v_row_bytes;
+  int v_ring_bytes;         // staging ring of the mover: a whole number of rows (tc_ring_bytes)
 };
 
 // ---- schedule: CTA c owns flattened units [c*U/nC, (c+1)*U/nC) -----------------------------------
@@ -79,20 +81,29 @@ struct TcSmem {
   uint8_t* k;        // K ring: [stage][2 halves][128 tokens][128 B]
   float* c;          // [512] per-row c_r (pass 2)
   float4* xch;       // [2][8][32] pass-1 exchange between the two token-half warps of a row block quarter
-  uint8_t* ring;     // V mover staging (kTcMoverRing bytes; only when a compaction is pending)
+  uint8_t* ring;     // V mover staging (v_ring_bytes; only when a compaction is pending)
   float2* xch2;      // [2][2][32] pass-1 exchange between the even- / odd-tile lane quarters of a half-full row block
   uint64_t* bars;    // mbarriers
   uint32_t* tmem;    // TMEM base address written by tcgen05.alloc
 };
-__host__ __device__ inline int tc_smem_bytes(int q_half_bytes, int n_kst, bool mover) {
-  return (mover ? kTcMoverRing : 0) + 1024 + 2 * q_half_bytes + n_kst * kTcKStage + kTcRowsMax * 4 + 8192 + 1024 + 256 + 16;
+__host__ __device__ inline int tc_smem_bytes(int q_half_bytes, int n_kst, int ring_bytes) {
+  return ring_bytes + 1024 + 2 * q_half_bytes + n_kst * kTcKStage + kTcRowsMax * 4 + 8192 + 1024 + 256 + 16;
+}
+// Staging ring of the V mover: what is left beside the Q rows and a 2-stage K ring, in whole rows, <= 32 rows and <= 32 KB;
+// 0 = fewer than kTcMoverRowsMin rows fit (the move then goes through k_gather).
+__host__ __device__ inline int tc_ring_bytes(int q_half_bytes, int row_bytes) {
+  const int avail = kTcSmemMax - tc_smem_bytes(q_half_bytes, 2, 0);
+  int rows = avail / row_bytes;
+  if (rows > 32) rows = 32;
+  if (rows * row_bytes > kTcMoverRingMax) rows = kTcMoverRingMax / row_bytes;
+  return rows >= kTcMoverRowsMin ? rows * row_bytes : 0;
 }
 __device__ inline TcSmem tc_carve(uint8_t* raw, const TcArgs& a) {
   uint8_t* p = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(raw) + 1023) & ~uintptr_t(1023));
   TcSmem s;
   s.q = p; p += 2 * a.q_half_bytes;
   s.k = p; p += a.n_kst * kTcKStage;
-  s.ring = p; p += a.v_base ? kTcMoverRing : 0;
+  s.ring = p; p += a.v_ring_bytes;
   s.c = reinterpret_cast<float*>(p); p += kTcRowsMax * 4;
   s.xch = reinterpret_cast<float4*>(p); p += 8192;
   s.xch2 = reinterpret_cast<float2*>(p); p += 1024;
@@ -517,7 +528,7 @@ __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const
 __device__ inline void tc_v_mover(const TcSmem& s, const TcBars& b, const TcArgs& a) {
   const int lane = threadIdx.x & 31;
   const int budget = a.g.budget, rb = a.v_row_bytes;
-  const int per = min(32, kTcMoverRing / rb);                             // rows per batch
+  const int per = a.v_ring_bytes / rb;                                    // rows per batch (8..32)
   const long long n_rows = (long long)a.g.B * a.g.L * budget;
   const long long r0 = n_rows * blockIdx.x / gridDim.x, r1 = n_rows * (blockIdx.x + 1) / gridDim.x;
   int bl = int(r0 / budget), sl = int(r0 - (long long)bl * budget) + lane;   // this lane's (slab, slot); no division below
@@ -659,10 +670,11 @@ inline bool tc_v_ride_ok(const hermes_t* h, int Tn, int P) {
   int n_sc = (R + kTcRowsMax - 1) / kTcRowsMax;
   const int RS = ((R + n_sc - 1) / n_sc + 31) & ~31;
   const int q_half = (RS + 63) / 64 * 8192;
-  if ((kTcSmemMax - tc_smem_bytes(q_half, 0, true)) / kTcKStage < 2) return false;
+  const int ring = tc_ring_bytes(q_half, int(h->lay.row_bytes));
+  if (ring == 0) return false;
   const double score_us = 2.0 * g.Hq * P * double(Tn) * (g.L - g.n_shallow) * g.B / 2.75e6;
   const double rows_per_cta = double(g.B) * g.L * g.budget / st->n_sm;
-  const double per = std::min<double>(32.0, double(kTcMoverRing) / double(h->lay.row_bytes));
+  const double per = double(ring / int(h->lay.row_bytes));
   return score_us >= 1.25 * (rows_per_cta / per * 3.0);
 }
 
@@ -704,9 +716,11 @@ inline int tc_score(hermes_t* h, const void* q_probe, int Tn, int P, float scale
   // a pending V compaction of the previous update rides in this launch (tc_v_mover)
   a.v_base = move_v ? static_cast<const char*>(g.vc) : nullptr;
   a.v_kept = g.kept; a.v_src_buf = h->v_src_buf; a.v_row_bytes = int(h->lay.row_bytes);
-  a.n_kst = std::min(kTcKStagesMax, (kTcSmemMax - tc_smem_bytes(a.q_half_bytes, 0, move_v)) / kTcKStage);
+  a.v_ring_bytes = move_v ? tc_ring_bytes(a.q_half_bytes, a.v_row_bytes) : 0;
+  if (move_v && a.v_ring_bytes == 0) { h->err = "internal: V mover ring does not fit (tc_v_ride_ok)"; return HERMES_ESTATE; }
+  a.n_kst = std::min(kTcKStagesMax, (kTcSmemMax - tc_smem_bytes(a.q_half_bytes, 0, a.v_ring_bytes)) / kTcKStage);
   if (a.n_kst < 2) { h->err = "tcgen05 scoring: shared memory too small for the K ring"; return HERMES_ESTATE; }
-  const int smem = tc_smem_bytes(a.q_half_bytes, a.n_kst, move_v);
+  const int smem = tc_smem_bytes(a.q_half_bytes, a.n_kst, a.v_ring_bytes);
   {
     TcProf p(h, HERMES_K_SCORE_STATS, s);
     // cooperative: pass 2 of a CTA waits for pass-1 statistics of other CTAs, so all of them must be resident
