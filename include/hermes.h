@@ -201,6 +201,29 @@ void hermes_destroy(hermes_t *h);
 /* Message of the last failing call on this handle (or of the last failing hermes_create if h == NULL). */
 const char *hermes_last_error(const hermes_t *h);
 
+/* ---- allocation-free Top-K (csrc/hermes_noalloc.cu) --------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it): Eq. 6 on ONE score vector, with no handle and no workspace.  Its scratch (268 KB: sortable
+ * keys, digit histograms, scan prefixes) is a file-scope static device array that every GPU loading the library holds
+ * until the process exits, hence the size limit below.
+ *   scores   : device, [n_tokens] fp32 (e.g. hermes_cache_view.last_scores); not modified.
+ *   kept_out : device, [k] int32; receives the indices of the k largest scores in ASCENDING index order.  Total order
+ *              (score, index): among equal scores the smaller index is evicted first -- the rule of the update path,
+ *              so for the same scores the result equals hermes_cache_view.last_kept bit for bit.
+ * Runs on the CURRENT device (cudaSetDevice); `cuda_stream` must belong to it.  Asynchronous: one kernel is enqueued.
+ * Errors: HERMES_EINVAL (NULL pointer, n_tokens < 1, k outside [1, n_tokens]); HERMES_ECAPACITY (n_tokens above the
+ * maximum of 65 536 reported by the max_tokens query below); HERMES_ECUDA (CUDA call failed).  The message is
+ * thread-local and read with the error query below.
+ * The call allocates nothing on host or device.  The first call on a device resolves the array's device address
+ * (cudaGetSymbolAddress, once per device); callers that capture graphs make that happen before capture with the
+ * setup call, on the device they will use.
+ * Every call on a GPU shares the one array: calls ordered on a stream (or by events) are safe, calls that OVERLAP on
+ * the GPU race on it and return garbage.                                                                           */
+int hermes_topk_noalloc(const float *scores, int32_t n_tokens, int32_t k, int32_t *kept_out, void *cuda_stream);
+int hermes_topk_noalloc_setup(void);           /* resolve the scratch address on the current device; HERMES_OK / _ECUDA */
+int32_t hermes_topk_noalloc_max_tokens(void);  /* 65536 */
+const char *hermes_topk_noalloc_error(void);   /* message of this thread's last failing no-alloc call ("" if none)    */
+
 #ifdef __cplusplus
 }
 #endif

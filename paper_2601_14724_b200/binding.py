@@ -23,7 +23,8 @@ HERMES_K_NAMES = ("append", "score_stats", "score_combine", "score_colsum", "sel
 EXPORTS = ("hermes_default_config", "hermes_workspace_bytes", "hermes_create", "hermes_append_chunk",
            "hermes_append_chunk_host", "hermes_get_cache", "hermes_len", "hermes_layer_len", "hermes_layer_budget", "hermes_layer_budgets", "hermes_device_status",
            "hermes_set_profiling", "hermes_get_profile", "hermes_last_score_path", "hermes_v_pending",
-           "hermes_last_launch_count", "hermes_destroy", "hermes_last_error")
+           "hermes_last_launch_count", "hermes_destroy", "hermes_last_error",
+           "hermes_topk_noalloc", "hermes_topk_noalloc_setup", "hermes_topk_noalloc_max_tokens", "hermes_topk_noalloc_error")
 
 
 class HermesConfig(C.Structure):
@@ -90,6 +91,12 @@ def load_library(rebuild_if_stale: bool = True) -> C.CDLL:
     lib.hermes_destroy.restype = None
     lib.hermes_last_error.argtypes = [vp]
     lib.hermes_last_error.restype = C.c_char_p
+    lib.hermes_topk_noalloc.argtypes = [vp, i32, i32, vp, vp]
+    lib.hermes_topk_noalloc_setup.argtypes = []
+    lib.hermes_topk_noalloc_max_tokens.argtypes = []
+    lib.hermes_topk_noalloc_max_tokens.restype = i32
+    lib.hermes_topk_noalloc_error.argtypes = []
+    lib.hermes_topk_noalloc_error.restype = C.c_char_p
     _lib = lib
     return lib
 
@@ -281,3 +288,32 @@ def hermes_destroy(h: Handle):
         load_library().hermes_destroy(h.ptr)
         h.ptr = None
         h.workspace = None
+
+
+# ---- allocation-free Top-K (csrc/hermes_noalloc.cu): no handle, no workspace, scratch in a static device array ----
+def hermes_topk_noalloc_max_tokens() -> int:
+    return int(load_library().hermes_topk_noalloc_max_tokens())
+
+
+def _noalloc_check(rc: int):
+    if rc != HERMES_OK:
+        msg = load_library().hermes_topk_noalloc_error()
+        raise HermesError(rc, msg.decode() if msg else "")
+
+
+def hermes_topk_noalloc_setup():
+    """Resolves the static scratch address on the current CUDA device (do this before graph capture)."""
+    _noalloc_check(load_library().hermes_topk_noalloc_setup())
+
+
+def hermes_topk_noalloc(scores, k: int, kept_out, stream=None):
+    """scores: contiguous fp32 device tensor [T]; kept_out: contiguous int32 device tensor [k] (caller-allocated).
+    Enqueues one kernel on `stream` of the CURRENT device; nothing is allocated.  The pointers are passed as they are:
+    the C entry point validates sizes (T > hermes_topk_noalloc_max_tokens() -> HERMES_ECAPACITY)."""
+    if scores.dtype != torch.float32 or not scores.is_cuda or not scores.is_contiguous() or scores.dim() != 1:
+        raise ValueError("scores must be a contiguous 1-D fp32 CUDA tensor")
+    if kept_out.dtype != torch.int32 or not kept_out.is_cuda or not kept_out.is_contiguous() or kept_out.numel() < max(k, 0):
+        raise ValueError("kept_out must be a contiguous int32 CUDA tensor with at least k elements")
+    rc = load_library().hermes_topk_noalloc(C.c_void_p(scores.data_ptr()), int(scores.numel()), int(k),
+                                            C.c_void_p(kept_out.data_ptr()), _stream_ptr(stream))
+    _noalloc_check(rc)

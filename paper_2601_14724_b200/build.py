@@ -26,11 +26,13 @@ def needs_build() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile csrc/hermes_api.cu -> libhermes_b200.so.  Raises if nvcc fails."""
+    """Compile csrc/*.cu (hermes_api.cu: the update path; hermes_noalloc.cu: the allocation-free Top-K) -> libhermes_b200.so.
+    Raises if nvcc fails."""
     if not force and not needs_build():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc, *NVCC_FLAGS, *os.environ.get("HERMES_NVCC_EXTRA", "").split(), "-o", LIB, os.path.join(CSRC, "hermes_api.cu")]
+    cmd = [nvcc, *NVCC_FLAGS, *os.environ.get("HERMES_NVCC_EXTRA", "").split(), "-o", LIB,
+           *[os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith(".cu")]]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     r = subprocess.run(cmd, capture_output=True, text=True)
