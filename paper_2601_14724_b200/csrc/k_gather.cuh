@@ -3,6 +3,11 @@
 // current buffer into the other one.  HBM-bound: every thread moves 4 x 16 bytes per step (K lo/hi halves
 // of a rotary pair group + the same two vectors of V), 128-bit coalesced, streaming cache policy; the
 // kept index and the position deltas of the NEXT step are prefetched while the current one is in flight.
+// Measured and not adopted (configs[1], K-only launch 68 us, pure copy under lazy re-indexing 57 us): table row requested
+// before the keys are unpacked (spills at 64 registers: 78 us); keys staged one trip ahead through thread-private shared
+// memory by cp.async (85 us; pure copy 68); rows moved by 1D bulk copies through a shared-memory ring and rotated in place
+// (79 us with the table read by __ldg, 111 us with the table row bulk-copied beside the key row; pure copy 56 us);
+// prefetch.global.L1 of the next trip's table slice (CCTL.PF1: 2 x slower).
 //
 // A "unit" = kPerVec rotary pairs of one KV head: elements [j0, j0+kPerVec) and [j0+d/2, ...) of the head.
 // Rotation: angle table (cos, sin)(delta * theta_j) built in fp64 at create time; fp32 products and
@@ -96,65 +101,52 @@ k_gather(Geom g, int cur) {
   const int32_t* kept = g.kept + size_t(bl) * g.budget;
   const int32_t* delta = g.delta + size_t(bl) * g.n_axes * g.budget;   // written by k_select
 
-  // units per trip: 1 everywhere.  (K-only mode with 2-4 units per trip, or with 5-6 blocks per SM, measured slower:
-  // 81-99 us against 72 us -- register spills at 64 registers, fewer resident blocks above that.)
-  constexpr int UPT = 1;
+  // One unit per thread and trip (K-only mode with 2-4 units per trip, or with 5-6 blocks per SM, measured slower: 81-99 us
+  // against 72 us -- register spills at 64 registers, fewer resident blocks above that).  A thread's unit index advances by
+  // `stride` per trip; its (row, unit in row) pair advances by (stride / upr, stride % upr) with a carry -- no integer
+  // division inside the loop (each costs ~25 instructions and a MUFU.RCP round trip in the dependent chain of the next loads).
+  const int rows = total / upr;
   const int stride = gridDim.x * kGatherThreads;
-  int idx[UPT], s[UPT], src[UPT], dl[UPT][NAX];
+  const int ds = stride / upr, du = stride - ds * upr;
+  const int sh = __ffs(uph) - 1;                            // uph = (d / 2) / V is a power of two (d is 32, 64 or 128)
+  int idx = blockIdx.x * kGatherThreads + threadIdx.x;
+  if (idx >= total) return;
+  int s = idx / upr, u = idx - s * upr;
+  int src = __ldcg(kept + s), dl[NAX];
 #pragma unroll
-  for (int p = 0; p < UPT; ++p) {
-    idx[p] = blockIdx.x * kGatherThreads + threadIdx.x + p * stride;
-    s[p] = min(idx[p], total - 1) / upr;
-    src[p] = __ldcg(kept + s[p]);
-#pragma unroll
-    for (int a = 0; a < NAX; ++a) dl[p][a] = __ldcg(delta + a * g.budget + s[p]);
-  }
-  if (idx[0] >= total) return;
+  for (int a = 0; a < NAX; ++a) dl[a] = __ldcg(delta + a * g.budget + s);
 
 #pragma unroll 1
   while (true) {
-    uint4 klo[UPT], khi[UPT], vlo[UPT], vhi[UPT];
-    int e[UPT], j0[UPT];
+    const int j0 = (u & (uph - 1)) * V, e = (u >> sh) * g.d + j0;
+    const size_t so = size_t(max(src, 0)) * g.row_elems + e;   // src < 0: the summary-token slot, written by k_summary
+    uint4 klo, khi, vlo, vhi;
+    klo = khi = vlo = vhi = make_uint4(0, 0, 0, 0);
+    if (kMode != kGatherV) { klo = ldg_stream(ks + so); khi = ldg_stream(ks + so + half); }
+    if (kMode != kGatherK) { vlo = ldg_stream(vs + so); vhi = ldg_stream(vs + so + half); }
+    // the next trip's position, row index and deltas (prefetched while this trip's vectors are in flight)
+    const int idx_n = idx + stride;
+    int s_n = s + ds, u_n = u + du;
+    if (u_n >= upr) { u_n -= upr; ++s_n; }
+    const int s_ld = min(s_n, rows - 1);
+    const int src_n = __ldcg(kept + s_ld);
+    int dl_n[NAX];
 #pragma unroll
-    for (int p = 0; p < UPT; ++p) {
-      const int u = min(idx[p], total - 1) - s[p] * upr;
-      e[p] = (u / uph) * g.d + (u % uph) * V;
-      j0[p] = (u % uph) * V;
-      const size_t so = size_t(max(src[p], 0)) * g.row_elems + e[p];   // src < 0: the summary-token slot, written by k_summary
-      klo[p] = khi[p] = vlo[p] = vhi[p] = make_uint4(0, 0, 0, 0);
-      if (kMode != kGatherV) { klo[p] = ldg_stream(ks + so); khi[p] = ldg_stream(ks + so + half); }
-      if (kMode != kGatherK) { vlo[p] = ldg_stream(vs + so); vhi[p] = ldg_stream(vs + so + half); }
+    for (int a = 0; a < NAX; ++a) dl_n[a] = __ldcg(delta + a * g.budget + s_ld);
+
+    bool any = false;
+#pragma unroll
+    for (int a = 0; a < NAX; ++a) any |= dl[a] != 0;
+    if (kMode != kGatherV && any) rotate_unit<T, NAX>(g, dl, j0, klo, khi);
+    const size_t dof = size_t(s) * g.row_elems + e;
+    if (src >= 0) {
+      if (kMode != kGatherV) { stg_stream(kd + dof, klo); stg_stream(kd + dof + half, khi); }
+      if (kMode != kGatherK) { stg_stream(vd + dof, vlo); stg_stream(vd + dof + half, vhi); }
     }
-    // prefetch the next trip's row indices and deltas
-    int idx_n[UPT], s_n[UPT], src_n[UPT], dl_n[UPT][NAX];
+    if (idx_n >= total) break;
+    idx = idx_n; s = s_n; u = u_n; src = src_n;
 #pragma unroll
-    for (int p = 0; p < UPT; ++p) {
-      idx_n[p] = idx[p] + UPT * stride;
-      s_n[p] = min(idx_n[p], total - 1) / upr;
-      src_n[p] = __ldcg(kept + s_n[p]);
-#pragma unroll
-      for (int a = 0; a < NAX; ++a) dl_n[p][a] = __ldcg(delta + a * g.budget + s_n[p]);
-    }
-#pragma unroll
-    for (int p = 0; p < UPT; ++p) {
-      if (idx[p] >= total) continue;
-      bool any = false;
-#pragma unroll
-      for (int a = 0; a < NAX; ++a) any |= dl[p][a] != 0;
-      if (kMode != kGatherV && any) rotate_unit<T, NAX>(g, dl[p], j0[p], klo[p], khi[p]);
-      const size_t dof = size_t(s[p]) * g.row_elems + e[p];
-      if (src[p] >= 0) {
-        if (kMode != kGatherV) { stg_stream(kd + dof, klo[p]); stg_stream(kd + dof + half, khi[p]); }
-        if (kMode != kGatherK) { stg_stream(vd + dof, vlo[p]); stg_stream(vd + dof + half, vhi[p]); }
-      }
-    }
-    if (idx_n[0] >= total) break;
-#pragma unroll
-    for (int p = 0; p < UPT; ++p) {
-      idx[p] = idx_n[p]; s[p] = s_n[p]; src[p] = src_n[p];
-#pragma unroll
-      for (int a = 0; a < NAX; ++a) dl[p][a] = dl_n[p][a];
-    }
+    for (int a = 0; a < NAX; ++a) dl[a] = dl_n[a];
   }
 }
 
