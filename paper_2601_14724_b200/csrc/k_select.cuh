@@ -209,7 +209,8 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
         const uint32_t key = orderable(s_sc[i]);
         if ((key & himask) == prefix) digit = (key >> shift) & 255u;
       }
-      // warp-private histogram: the shared-memory atomics only ever collide inside one warp
+      // warp-private histogram: the shared-memory atomics only ever collide inside one warp (aggregating equal digits with
+      // __match_any_sync first, one add per group, measured slower: wsum + select 24 -> 30 us, 59 -> 91 us at T = 32 964)
       if (digit != 0xFFFFFFFFu) atomicAdd(&my_hist[digit], 1);
     }
     __syncthreads();
