@@ -189,20 +189,30 @@ def run_ours(args, backend=None, hb=None):
         over.update(summary_token=1)
     if args.no_defer_v:
         over.update(defer_v=0)
+    lb = None
+    if args.budget_weight:                                   # layer-dependent budgets (Tab. 5)
+        lb = tuple(float(x) for x in args.budget_weight.split(","))
+        assert len(lb) == 3, "--budget-weight takes shallow,middle,deep"
+        over.update(budget_weight=lb, max_tokens=0)
     cfg = hb.config_for_workload(wl, device=local_rank, **over)
     h = hb.hermes_create(cfg)
+    fill_to = max(hb.hermes_layer_budgets(cfg)) if lb else wl.budget   # every layer holds at least its budget before timing
 
     host_pool = [tuple(be.pin(torch.from_numpy(x).to(tdt)) for x in s) for s in make_pool(wl, rank, POOL)]
     dev_pool = [tuple(x.to(dev) for x in s) for s in host_pool]
     # fill to the budget without a probe (no eviction), then W warm evicting updates
-    n_fill, rem = divmod(wl.budget, wl.chunk_tokens)
-    for i in range(n_fill):
-        K, V, _ = dev_pool[i % POOL]
-        hb.hermes_append_chunk(h, K, V, None)
-    if rem:                                                  # budget not a multiple of the chunk: one partial append
-        K, V, _ = dev_pool[n_fill % POOL]
-        hb.hermes_append_chunk(h, K[:, :, :rem].contiguous(), V[:, :, :rem].contiguous(), None)
-    assert hb.hermes_len(h) == wl.budget
+    n_fill, rem = divmod(fill_to, wl.chunk_tokens)
+
+    def fill(hh):
+        for i in range(n_fill):
+            K, V, _ = dev_pool[i % POOL]
+            hb.hermes_append_chunk(hh, K, V, None)
+        if rem:                                              # budget not a multiple of the chunk: one partial append
+            K, V, _ = dev_pool[n_fill % POOL]
+            hb.hermes_append_chunk(hh, K[:, :, :rem].contiguous(), V[:, :, :rem].contiguous(), None)
+        assert hb.hermes_len(hh) == fill_to
+
+    fill(h)
 
     def barrier():
         be.synchronize()
@@ -253,7 +263,8 @@ def run_ours(args, backend=None, hb=None):
 
     def host_step(i):
         K, V, Q = host_pool[i % POOL]
-        hb.hermes_append_chunk_host(h, K, V, Q, kept_out=kept_host[i & 1])
+        # (with layer-dependent budgets the lists have per-layer lengths and the host entry point does not return them)
+        hb.hermes_append_chunk_host(h, K, V, Q, kept_out=None if lb else kept_host[i & 1])
         replay.append(i % POOL)
         done[i & 1] = be.event()
         done[i & 1].record()
@@ -265,7 +276,8 @@ def run_ours(args, backend=None, hb=None):
         host_step(i)
     ms_e2e = timed(n_e2e, host_step)
     h2d = sum(x.numel() * x.element_size() for x in host_pool[0])
-    d2h = kept_host[0].numel() * 4
+    d2h = 0 if lb else kept_host[0].numel() * 4
+    rides = bool(hb.hermes_v_pending(h))
 
     # outside every timed region: the cache the timed updates left behind must equal, bit for bit, the cache of a
     # handle that never defers a compaction (defer_v = 0; that configuration is the one the lock-step
@@ -273,12 +285,7 @@ def run_ours(args, backend=None, hb=None):
     check = None
     if not args.no_replay_check:
         h2 = hb.hermes_create(hb.config_for_workload(wl, device=local_rank, **dict(over, defer_v=0)))
-        for i in range(n_fill):
-            K, V, _ = dev_pool[i % POOL]
-            hb.hermes_append_chunk(h2, K, V, None)
-        if rem:
-            K, V, _ = dev_pool[n_fill % POOL]
-            hb.hermes_append_chunk(h2, K[:, :, :rem].contiguous(), V[:, :, :rem].contiguous(), None)
+        fill(h2)
         for j in replay:
             K, V, Q = dev_pool[j]
             hb.hermes_append_chunk(h2, K, V, Q)
@@ -324,7 +331,7 @@ def run_ours(args, backend=None, hb=None):
                     exp2={"peak_gexp2_s": xu_peak, "method_gexp2_s": n_exp_method / t_dom / 1e9, "method_frac": n_exp_method / t_dom / 1e9 / xu_peak,
                           "design_gexp2_s": 2 * n_exp_method / t_dom / 1e9, "design_frac": 2 * n_exp_method / t_dom / 1e9 / xu_peak,
                           "note": "XU pipe, 16 exp2/clk/SM x 148 SMs x clocks.max.sm; the design evaluates 2 exp2 per (probe row, token)"},
-                    rides="the previous update's V compaction (360 MB) is moved inside this launch")
+                    rides="the previous update's V compaction is moved inside this launch" if rides else None)
     elif dom in ("score_stats", "score_colsum"):
         ach = work["flops"] / t_dom / 1e12
         roof = dict(kernel=dom, bound="tensor", achieved=ach, peak=pk["tensor"], unit="TFLOP/s", frac=ach / pk["tensor"], traffic=traffic)
@@ -351,7 +358,8 @@ def run_ours(args, backend=None, hb=None):
                    "l2": (f"cache slabs touched per step: {ws_mb:.0f} MB read + {wr_mb:.0f} MB written "
                           + ("(exceeds the 126 MB L2)" if ws_mb + wr_mb > 252 else "(comparable to the 126 MB L2: no flush, L2-assisted)")
                           + f"; inputs cycle through {POOL} chunk/probe sets"),
-                   "score_path": score_path, "reindex": args.reindex, "summary_token": bool(args.summary_token)},
+                   "score_path": score_path, "reindex": args.reindex, "summary_token": bool(args.summary_token),
+                   **({"budget_weight": list(lb), "layer_budgets_min_max": [min(hb.hermes_layer_budgets(cfg)), max(hb.hermes_layer_budgets(cfg))]} if lb else {})},
         "e2e": {"value": job_value(wl, world, B, ms_e2e), "unit": UNIT, "ms_per_step": ms_e2e,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e},
         "gpu_launches": launches,
@@ -424,6 +432,7 @@ def main():
     ap.add_argument("--reindex", default="eager", choices=["eager", "lazy"])
     ap.add_argument("--max-position", type=int, default=32768, help="lazy re-indexing: the model's position limit")
     ap.add_argument("--summary-token", action="store_true")
+    ap.add_argument("--budget-weight", default="", help="layer-dependent budgets: shallow,middle,deep weights (PAPER.md Tab. 5), e.g. 1.3,1.0,0.7")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-defer-v", action="store_true", help="compact V in the gather kernel instead of inside the next scoring launch")
     ap.add_argument("--no-replay-check", action="store_true", help="skip the post-timing bit-equality check against a non-deferring handle")

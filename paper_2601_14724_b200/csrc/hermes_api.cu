@@ -208,7 +208,7 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
     return HERMES_ECUDA;
   }
   // tensor-core scoring path: bf16, d = 128; probing it builds its tensor maps
-  h->tc_ok = !h->lb && tc_init(h);                 // layer-dependent budgets score on the CUDA-core path
+  h->tc_ok = tc_init(h);
   if (c->score_path == HERMES_SCORE_TCGEN05 && !h->tc_ok) {
     std::string why = h->err;
     delete h;
@@ -421,12 +421,16 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
   for (bool& r : h->timer.ran) r = false;
   const int row_vecs = int(h->lay.row_bytes / 16);
   const int BL = g.B * g.L;
+  // tokens the scoring launch spans: with layer-dependent budgets the largest SCORED layer's candidates (k_tc_score<true>
+  // masks the rest per layer); shallow layers, which may hold more, are not scored
+  int Tn_sc = Tn;
+  if (h->lb) { Tn_sc = 1; for (int l = g.n_shallow; l < c.n_layers; ++l) Tn_sc = std::max(Tn_sc, int(dyn[l])); }
   const bool use_tc = evict && g.L > g.n_shallow && h->tc_ok && c.score_path != HERMES_SCORE_SIMT &&
-                      (c.score_path == HERMES_SCORE_TCGEN05 || tc_profitable(h, Tn, n_probe));
+                      (c.score_path == HERMES_SCORE_TCGEN05 || tc_profitable(h, Tn_sc, n_probe));
   h->last_stream = cuda_stream;
   // a pending V compaction rides in this update's scoring kernel if that kernel is long enough and has the
   // shared memory for it; otherwise it runs on its own first
-  const bool ride = use_tc && tc_v_ride_ok(h, Tn, n_probe);
+  const bool ride = use_tc && !h->lb && tc_v_ride_ok(h, Tn, n_probe);   // the mover assumes `budget` rows per slab
   if (!ride) flush_v(h, s);
   {
     Prof p(h, HERMES_K_APPEND, s);
@@ -451,7 +455,7 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
     if (g.L > g.n_shallow) {
       bool scored = false;
       if (use_tc) {
-        const int rc = tc_score(h, Q_probe, Tn, n_probe, scale_log2, s, ride && h->v_pending);
+        const int rc = tc_score(h, Q_probe, Tn_sc, n_probe, scale_log2, s, ride && h->v_pending);
         if (rc == kTcNotResident) {
           // the device cannot hold one scoring CTA per unit of its grid at once (MPS / green-context partition): this
           // handle scores on the CUDA-core path from now on; a pending V compaction runs on its own

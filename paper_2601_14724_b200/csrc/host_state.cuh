@@ -98,7 +98,6 @@ inline const char* validate(const hermes_config& c) {
   for (float w : c.budget_weight) if (!(w > 0.f) || !std::isfinite(w)) return "budget_weight must be positive";
   if (!uniform_budgets(c)) {
     if (c.rope_mode != HERMES_ROPE_1D || c.summary_token) return "layer-dependent budgets need 1D RoPE and no summary token";
-    if (c.score_path == HERMES_SCORE_TCGEN05) return "layer-dependent budgets score on the CUDA-core path";
     for (int m : layer_budgets(c, ns, nd)) {
       if (m < 1) return "a layer's budget would be zero";
       if (c.max_tokens != 0 && c.max_tokens <= m) return "max_tokens must exceed the largest layer budget (or be 0)";

@@ -187,7 +187,7 @@ __device__ inline void tc_producer(const TcSmem& s, const TcBars& b, const CUten
 // A TMEM stage (256 columns) holds a "half-group" = 2 row blocks x 128 tokens; epilogue warp
 // (row block rbl, 64-token half th, lane quarter lg) takes its 64 columns as two 32-column blocks.
 // =====================================================================================================
-template <bool kEpi>
+template <bool kEpi, bool kLb>
 __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const CUtensorMap* tmap_q, const CUtensorMap* tmap_k,
                                          const TcArgs& a, uint32_t tmem_base, TcRole& st) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -281,6 +281,11 @@ __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const
     };
     int x = s0 % a.spg, gi = s0 / a.spg, n_done = 0;
     TcCursor g; g.init(a, gi);
+    // candidates of the group's layer: a.Tn, or (kLb) this layer's own count under layer-dependent budgets (DESIGN f4): the
+    // tile grid is the largest scored layer's, tokens past T_l are masked like the ragged tail of the last tile.  A template
+    // flag, not a run-time test: one more live register in this loop spills (+2 us at configs[1])
+    int T_l = a.Tn;
+    if (kLb) T_l = layer_T(a.g, g.bl(a) % a.g.L, a.Tn);
     // tell pass 2 (of this or a neighbouring CTA) that `n_done` more segments of group gi are in memory
     auto publish = [&]() {
       __threadfence();
@@ -297,7 +302,7 @@ __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const
       const bool act1_odd = lg >= 2 && 384 + (lg - 2) * 32 < rs_valid;
       const int t_end = min(a.tpg, (x + 1) * kTcSegTiles);
       for (int t = x * kTcSegTiles; t < t_end; ++t) {
-        const int n_valid = a.Tn - (t * kTcTile + th * 64);
+        const int n_valid = T_l - (t * kTcTile + th * 64);
 #pragma unroll
         for (int hg = 0; hg < 2; ++hg) {
           if (hg == 1 && !two) break;
@@ -342,15 +347,15 @@ __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const
             ptx::named_bar_sync(10 + (lg & 1), 64);
             if (lg < 2 && row_b < rs_valid) {
               const float2 o = *x2;
-              const float m = fmaxf(mb, o.x);                            // a segment holds at least one tile: not both -inf
-              part[row_b] = make_float2(m, zb * fast_exp2(mb - m) + o.y * fast_exp2(o.x - m));
+              const float m = fmaxf(mb, o.x);                            // both -inf: a segment past this layer's candidates
+              part[row_b] = make_float2(m, m == -INFINITY ? 0.f : zb * fast_exp2(mb - m) + o.y * fast_exp2(o.x - m));
             }
           }
         }
         m0 = m1 = -INFINITY; z0 = z1 = 0.f;
       }
       ++n_done;
-      if (++x == a.spg) { publish(); x = 0; ++gi; g.next(a); }
+      if (++x == a.spg) { publish(); x = 0; ++gi; g.next(a); if (kLb) T_l = layer_T(a.g, g.bl(a) % a.g.L, a.Tn); }
     }
     if (n_done > 0) publish();
     st.as = as; st.aph = aph;
@@ -394,7 +399,7 @@ __device__ __noinline__ void tc_merge_rows(const float2* pr, int n_slot, int row
 // holds a chunk of <= 256 probe rows of the 128-token tile; epilogue warp (lane quarter lg, column
 // quarter cq) takes 32-column blocks cq and cq + 4 of the chunk.
 // =====================================================================================================
-template <bool kEpi>
+template <bool kEpi, bool kLb>
 __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const CUtensorMap* tmap_q, const CUtensorMap* tmap_k,
                                          const TcArgs& a, uint32_t tmem_base, TcRole& st) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -450,7 +455,7 @@ __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const
     float v[32];
     float acc[4] = {0.f, 0.f, 0.f, 0.f};
     bool new_group = true;
-    int t = u0 % a.tpg, rs32 = 0, gi = u0 / a.tpg;
+    int t = u0 % a.tpg, rs32 = 0, gi = u0 / a.tpg, T_l = a.Tn;
     float* col = nullptr;                                                // this warp's column-sum slot of the group
     TcCursor g; g.init(a, gi);
     // seg_cnt[group] counts 16 (epilogue warps) per finished pass-1 segment of THIS update: k_append zeroes the counters
@@ -489,6 +494,7 @@ __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const
                       g.ls >= a.g.L - a.g.n_shallow - a.g.n_deep ? a.g.probe_deep_begin : 0);
         ptx::named_bar_sync(1, kTcEpiWarps * 32);
         rs32 = (g.rs_valid(a) + 31) & ~31;
+        if (kLb) T_l = layer_T(a.g, bl % a.g.L, a.Tn);
         col = a.g.colsum + (size_t(bl) * a.g.n_vh_max + (g.kvh * a.n_sc + g.sc) * 4 + cq) * a.g.cap;
         new_group = false;
       }
@@ -514,7 +520,7 @@ __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const
       }
       // per-(KV head, super-chunk, column quarter) column sum of this token; k_wsum adds the slots in order
       const int tok = t * kTcTile + tok_in_tile;
-      if (tok < a.Tn) col[tok] = (acc[0] + acc[1]) + (acc[2] + acc[3]);
+      if (tok < T_l) col[tok] = (acc[0] + acc[1]) + (acc[2] + acc[3]);
       acc[0] = acc[1] = acc[2] = acc[3] = 0.f;
       if (++t == a.tpg) { t = 0; ++gi; g.next(a); new_group = true; }
     }
@@ -565,6 +571,8 @@ __device__ inline void tc_v_mover(const TcSmem& s, const TcBars& b, const TcArgs
 // schedule neighbours -- there is no grid-wide barrier.  Requires every CTA resident: the launch is cooperative
 // (gridDim.x <= #SMs; the runtime refuses it on an SM-limited context, and the caller falls back to the CUDA-core path).
 // =====================================================================================================
+// kLb: layer-dependent budgets (per-layer candidate counts); the uniform-budget instantiation is the one bench.py times.
+template <bool kLb>
 __global__ void __launch_bounds__(kTcThreads, 1)
 k_tc_score(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k, TcArgs a) {
   extern __shared__ uint8_t smem_raw[];
@@ -579,12 +587,12 @@ k_tc_score(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ C
   if ((threadIdx.x >> 5) < kTcCtlWarps) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kTcRegsCtl));
     if ((threadIdx.x >> 5) == 2 && a.v_base != nullptr) tc_v_mover(s, b, a);
-    tc_pass1<false>(s, b, &tmap_q, &tmap_k, a, tmem_base, st);
-    tc_pass2<false>(s, b, &tmap_q, &tmap_k, a, tmem_base, st);
+    tc_pass1<false, kLb>(s, b, &tmap_q, &tmap_k, a, tmem_base, st);
+    tc_pass2<false, kLb>(s, b, &tmap_q, &tmap_k, a, tmem_base, st);
   } else {
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kTcRegsEpi));
-    tc_pass1<true>(s, b, &tmap_q, &tmap_k, a, tmem_base, st);
-    tc_pass2<true>(s, b, &tmap_q, &tmap_k, a, tmem_base, st);
+    tc_pass1<true, kLb>(s, b, &tmap_q, &tmap_k, a, tmem_base, st);
+    tc_pass2<true, kLb>(s, b, &tmap_q, &tmap_k, a, tmem_base, st);
   }
   ptx::tc_fence_before();
   __syncthreads();
@@ -641,8 +649,9 @@ inline bool tc_init(hermes_t* h) {
     h->err = "cuTensorMapEncodeTiled(K cache) failed"; delete st; return false;
   }
   int occ = 0;
-  if (cudaFuncSetAttribute(k_tc_score, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemMax) != cudaSuccess ||
-      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_tc_score, kTcThreads, kTcSmemMax) != cudaSuccess || occ < 1) {
+  if (cudaFuncSetAttribute(k_tc_score<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemMax) != cudaSuccess ||
+      cudaFuncSetAttribute(k_tc_score<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemMax) != cudaSuccess ||
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_tc_score<false>, kTcThreads, kTcSmemMax) != cudaSuccess || occ < 1) {
     h->err = std::string("cudaFuncSetAttribute(tc kernels): ") + cudaGetErrorString(cudaGetLastError());
     delete st; return false;
   }
@@ -724,7 +733,8 @@ inline int tc_score(hermes_t* h, const void* q_probe, int Tn, int P, float scale
   {
     TcProf p(h, HERMES_K_SCORE_STATS, s);
     // cooperative: pass 2 of a CTA waits for pass-1 statistics of other CTAs, so all of them must be resident
-    const cudaError_t e = launch_pdl_coop(k_tc_score, dim3(n_cta), dim3(kTcThreads), size_t(smem), s, tmap_q, st->tmap_k, a);
+    const cudaError_t e = h->lb ? launch_pdl_coop(k_tc_score<true>, dim3(n_cta), dim3(kTcThreads), size_t(smem), s, tmap_q, st->tmap_k, a)
+                                : launch_pdl_coop(k_tc_score<false>, dim3(n_cta), dim3(kTcThreads), size_t(smem), s, tmap_q, st->tmap_k, a);
     if (e == cudaErrorCooperativeLaunchTooLarge) {             // not every CTA can be resident (SM-limited context): no spin-waits then
       (void)cudaGetLastError();
       return kTcNotResident;

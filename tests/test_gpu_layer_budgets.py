@@ -41,6 +41,7 @@ def _run(wl, w, n_updates, **over):
     fd = Feeder(wl, 0)
     half = wl.head_dim // 2
     n_cmp = n_untouched = 0
+    paths = set()
     sizes = [wl.preload_tokens] if wl.preload_tokens else []
     for u, n in enumerate(sizes + [wl.chunk_tokens] * n_updates):
         st = _gpu_state(h, ocfg, wl)
@@ -49,6 +50,8 @@ def _run(wl, w, n_updates, **over):
         hb.hermes_append_chunk(h, to_dev(K[None], wl.dtype), to_dev(V[None], wl.dtype), None if Q is None else to_dev(Q[None], wl.dtype))
         torch.cuda.synchronize()
         out = ho.oracle_step_layer_budgets(st, K, V, Q)
+        if out["evicted"]:
+            paths.add(hb.hermes_last_score_path(h))
         assert hb.hermes_len(h) == int(st.lens.max())
         for l in range(wl.n_layers):
             v = hb.hermes_get_cache(h, 0, l)
@@ -82,28 +85,37 @@ def _run(wl, w, n_updates, **over):
                 tol = np.maximum(tol, 2 * bf16_ulp(ko))
             assert (np.abs(k_gpu.astype(np.float64) - ko) <= tol + 1e-30).all(), f"layer {l}: K beyond tolerance"
             n_cmp += 1
-    assert hb.hermes_device_status(h) == 0 and hb.hermes_last_score_path(h) == hb.HERMES_SCORE_SIMT
+    assert hb.hermes_device_status(h) == 0 and hb.hermes_v_pending(h) == 0
     lens = [hb.hermes_layer_len(h, l) for l in range(wl.n_layers)]
     hb.hermes_destroy(h)
-    return m, lens, n_cmp, n_untouched
+    return m, lens, n_cmp, n_untouched, paths
 
 
 @pytest.mark.parametrize("w", TAB5)
 def test_toy_config_at_tab5_weightings(w):
     wl = CONFIGS["toy"]                                       # fp32, 4 layers (1 / 2 / 1), preload 128, chunks of 32
-    m, lens, n_cmp, n_untouched = _run(wl, w, 8)
-    assert lens == m.tolist() and n_cmp >= 20
+    m, lens, n_cmp, n_untouched, paths = _run(wl, w, 8)
+    assert lens == m.tolist() and n_cmp >= 20 and paths == {hb.HERMES_SCORE_SIMT}
     if m.max() > 160:
         assert n_untouched > 0                                # a big layer was still under its budget while others compressed
 
 
 def test_bf16_geometry_at_tab5_weighting():
     wl = CONFIGS["llava_ov_7b"].scaled(n_layers=7, budget=588, probe_tokens=8)     # 1 / 4 / 2 layers, bf16, d 128
-    m, lens, n_cmp, _ = _run(wl, (0.7, 1.0, 1.3), 6)
-    assert lens == np.minimum(m, 196 * 6).tolist() and n_cmp >= 14
+    m, lens, n_cmp, _, paths = _run(wl, (0.7, 1.0, 1.3), 6, score_path=hb.HERMES_SCORE_SIMT)
+    assert lens == np.minimum(m, 196 * 6).tolist() and n_cmp >= 14 and paths == {hb.HERMES_SCORE_SIMT}
+
+
+@pytest.mark.parametrize("w", TAB5)
+def test_bf16_geometry_on_tcgen05_at_tab5_weightings(w):
+    """Per-layer candidate counts on the tensor-core scoring path (k_tc_score<true>): the tile grid is the largest scored
+    layer's, every other layer's tail -- whole tiles and whole pass-1 segments of it at these weightings -- is masked."""
+    wl = CONFIGS["llava_ov_7b"].scaled(n_layers=7, budget=896, probe_tokens=24)    # 1 / 4 / 2 layers; T_l from ~820 to ~1450
+    m, lens, n_cmp, _, paths = _run(wl, w, 10, score_path=hb.HERMES_SCORE_TCGEN05)
+    assert lens == np.minimum(m, 196 * 10).tolist() and n_cmp >= 20 and paths == {hb.HERMES_SCORE_TCGEN05}
 
 
 def test_equal_weights_are_the_uniform_path():
     wl = CONFIGS["toy"]
-    m, lens, n_cmp, n_untouched = _run(wl, (2.0, 2.0, 2.0), 3)
+    m, lens, n_cmp, n_untouched, _ = _run(wl, (2.0, 2.0, 2.0), 3)
     assert lens == [wl.budget] * wl.n_layers and n_untouched == 0
