@@ -99,7 +99,7 @@ typedef struct {
                                    layer.  With the total budget * n_layers fixed, layer i keeps
                                    m_i = floor(w_i / sum_j w_j * budget * n_layers) tokens, the residue goes to the last
                                    layer.  {1, 1, 1} (default): `budget` everywhere.  Unequal weights need HERMES_ROPE_1D
-                                   and no summary token; V is then compacted with K (no deferred move)           */
+                                   and no summary token                                                           */
   int32_t defer_v;              /* 1 (default): on the tcgen05 path an eviction compacts K at once but leaves the
                                    kept V rows to be moved by the NEXT update's scoring kernel (V is not read by
                                    scoring, so the copy hides behind it); hermes_get_cache() and updates that do

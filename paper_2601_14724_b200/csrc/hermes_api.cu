@@ -415,8 +415,6 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
   if (lazy && p0 + span > c.max_position) return fail(h, HERMES_ECAPACITY, "positions would exceed max_position %d", c.max_position);
 
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-  // stream-ordered behind the previous update's kernels; the source is pageable memory, so the call has staged it on return
-  if (h->lb) CUDA_TRY(h, cudaMemcpyAsync(h->ws + h->lay.lay_dyn, dyn.data(), dyn.size() * 4, cudaMemcpyHostToDevice, s));
   h->last_launches = 0;
   for (bool& r : h->timer.ran) r = false;
   const int row_vecs = int(h->lay.row_bytes / 16);
@@ -430,8 +428,11 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
   h->last_stream = cuda_stream;
   // a pending V compaction rides in this update's scoring kernel if that kernel is long enough and has the
   // shared memory for it; otherwise it runs on its own first
-  const bool ride = use_tc && !h->lb && tc_v_ride_ok(h, Tn, n_probe);   // the mover assumes `budget` rows per slab
+  const bool ride = use_tc && tc_v_ride_ok(h, Tn_sc, n_probe);
   if (!ride) flush_v(h, s);
+  // the per-layer tables of THIS update, stream-ordered behind the previous update's kernels and behind a flush (which reads
+  // the previous update's counts); the source is pageable memory, so the call has staged it on return
+  if (h->lb) CUDA_TRY(h, cudaMemcpyAsync(h->ws + h->lay.lay_dyn, dyn.data(), dyn.size() * 4, cudaMemcpyHostToDevice, s));
   {
     Prof p(h, HERMES_K_APPEND, s);
     const size_t n_vec = size_t(n_new) * row_vecs;
@@ -455,13 +456,21 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
     if (g.L > g.n_shallow) {
       bool scored = false;
       if (use_tc) {
-        const int rc = tc_score(h, Q_probe, Tn_sc, n_probe, scale_log2, s, ride && h->v_pending);
+        const int rc = tc_score(h, Q_probe, Tn_sc, n_new, n_probe, scale_log2, s, ride && h->v_pending);
         if (rc == kTcNotResident) {
           // the device cannot hold one scoring CTA per unit of its grid at once (MPS / green-context partition): this
           // handle scores on the CUDA-core path from now on; a pending V compaction runs on its own
           if (c.score_path == HERMES_SCORE_TCGEN05) return fail(h, HERMES_ECUDA, "tcgen05 scoring kernel cannot be made resident on this device partition");
           h->tc_ok = false;
-          flush_v(h, s);
+          if (h->lb && h->v_pending) {               // the flush counts rows with the PREVIOUS update's table: put it back for it
+            std::vector<int32_t> prev(dyn);
+            for (int l = 0; l < c.n_layers; ++l) prev[c.n_layers + l] = h->lay_len[l];
+            CUDA_TRY(h, cudaMemcpyAsync(h->ws + h->lay.lay_dyn, prev.data(), prev.size() * 4, cudaMemcpyHostToDevice, s));
+            flush_v(h, s);
+            CUDA_TRY(h, cudaMemcpyAsync(h->ws + h->lay.lay_dyn, dyn.data(), dyn.size() * 4, cudaMemcpyHostToDevice, s));
+          } else {
+            flush_v(h, s);
+          }
         } else if (rc != HERMES_OK) {
           return rc;
         } else {

@@ -52,6 +52,7 @@ struct TcArgs {
   const char* v_base;       // V cache base, or NULL: nothing pending
   const int32_t* v_kept;    // [B*L][budget] kept lists of the previous update
   int v_src_buf, v_row_bytes;
+  int v_n_new;              // layer-dependent budgets: rows layer l held after the previous update = lay_T[l] - v_n_new
   int v_ring_bytes;         // staging ring of the mover: a whole number of rows (tc_ring_bytes)
 };
 
@@ -538,12 +539,15 @@ __device__ inline void tc_v_mover(const TcSmem& s, const TcBars& b, const TcArgs
   const long long n_rows = (long long)a.g.B * a.g.L * budget;
   const long long r0 = n_rows * blockIdx.x / gridDim.x, r1 = n_rows * (blockIdx.x + 1) / gridDim.x;
   int bl = int(r0 / budget), sl = int(r0 - (long long)bl * budget) + lane;   // this lane's (slab, slot); no division below
+  int l = bl % a.g.L;
   int ph = 0;
   for (long long i0 = r0; i0 < r1; i0 += per) {
-    while (sl >= budget) { sl -= budget; ++bl; }
+    while (sl >= budget) { sl -= budget; ++bl; if (++l == a.g.L) l = 0; }
     const bool on = lane < per && i0 + lane < r1;
     int src = -1;
     if (on) src = __ldcg(a.v_kept + size_t(bl) * budget + sl);            // < 0: summary-token slot, not a copy
+    // layer-dependent budgets: `budget` is the list stride (the largest layer's); this layer holds fewer rows
+    if (on && a.g.lay_T != nullptr && sl >= __ldg(a.g.lay_T + l) - a.v_n_new) src = -1;
     const unsigned m = __ballot_sync(0xffffffffu, on && src >= 0);
     if (m != 0) {
       if (lane == 0) ptx::mbar_expect_tx(b.v_full, uint32_t(__popc(m)) * rb);
@@ -698,7 +702,7 @@ struct TcProf {   // same event bracketing as hermes_api.cu's Prof, local to thi
   ~TcProf() { if (h->profiling) cudaEventRecord(h->timer.end[id], s); }
 };
 
-inline int tc_score(hermes_t* h, const void* q_probe, int Tn, int P, float scale_log2, cudaStream_t s, bool move_v) {
+inline int tc_score(hermes_t* h, const void* q_probe, int Tn, int n_new, int P, float scale_log2, cudaStream_t s, bool move_v) {
   TcState* st = static_cast<TcState*>(h->tc_state);
   const Geom& g = h->geom;
   CUtensorMap tmap_q;
@@ -724,7 +728,7 @@ inline int tc_score(hermes_t* h, const void* q_probe, int Tn, int P, float scale
   a.q_half_bytes = (a.RS + 63) / 64 * 8192;
   // a pending V compaction of the previous update rides in this launch (tc_v_mover)
   a.v_base = move_v ? static_cast<const char*>(g.vc) : nullptr;
-  a.v_kept = g.kept; a.v_src_buf = h->v_src_buf; a.v_row_bytes = int(h->lay.row_bytes);
+  a.v_kept = g.kept; a.v_src_buf = h->v_src_buf; a.v_row_bytes = int(h->lay.row_bytes); a.v_n_new = n_new;
   a.v_ring_bytes = move_v ? tc_ring_bytes(a.q_half_bytes, a.v_row_bytes) : 0;
   if (move_v && a.v_ring_bytes == 0) { h->err = "internal: V mover ring does not fit (tc_v_ride_ok)"; return HERMES_ESTATE; }
   a.n_kst = std::min(kTcKStagesMax, (kTcSmemMax - tc_smem_bytes(a.q_half_bytes, 0, a.v_ring_bytes)) / kTcKStage);

@@ -119,3 +119,47 @@ def test_equal_weights_are_the_uniform_path():
     wl = CONFIGS["toy"]
     m, lens, n_cmp, n_untouched, _ = _run(wl, (2.0, 2.0, 2.0), 3)
     assert lens == [wl.budget] * wl.n_layers and n_untouched == 0
+
+
+def test_deferred_v_move_with_layer_budgets_full_size():
+    """configs[1] geometry at a Tab. 5 weighting, the launch bench.py --budget-weight times: consecutive evicting updates with
+    no hermes_get_cache in between, so the previous update's V compaction (per-layer row counts) rides in the scoring
+    launch.  The final cache must equal, bit for bit, that of a handle that never defers (the configuration the lock-step
+    tests above compare with the oracle)."""
+    wl = CONFIGS["llava_ov_7b"]
+    w = (1.3, 1.0, 0.7)
+    gen = torch.Generator(device="cuda").manual_seed(4242)
+    L, Hkv, Hq, d, C, P = wl.n_layers, wl.n_kv_heads, wl.n_q_heads, wl.head_dim, wl.chunk_tokens, wl.probe_tokens
+    chunks = [tuple(torch.randn(1, L, C, Hkv, d, generator=gen, device="cuda").to(torch.bfloat16) for _ in range(2)) +
+              (torch.randn(1, L, Hq, P, d, generator=gen, device="cuda").to(torch.bfloat16),) for _ in range(6)]
+    caches = []
+    for defer in (1, 0):
+        cfg = hb.config_for_workload(wl, budget_weight=w, max_tokens=0, defer_v=defer)
+        h = hb.hermes_create(cfg)
+        m_max = max(hb.hermes_layer_budgets(cfg))
+        n = 0
+        while hb.hermes_len(h) < m_max:                       # fill without a probe: nothing is evicted
+            K, V, _ = chunks[n % 6]
+            take = min(C, m_max - hb.hermes_len(h))
+            hb.hermes_append_chunk(h, K[:, :, :take].contiguous(), V[:, :, :take].contiguous(), None)
+            n += 1
+        pend = []
+        for i in range(5):
+            K, V, Q = chunks[i % 6]
+            hb.hermes_append_chunk(h, K, V, Q)
+            pend.append(hb.hermes_v_pending(h))
+        assert hb.hermes_last_score_path(h) == hb.HERMES_SCORE_TCGEN05
+        assert pend == [defer] * 5, pend                      # the move rides (and is pending again) at every update
+        torch.cuda.synchronize()
+        out = []
+        for l in range(L):
+            v = hb.hermes_get_cache(h, 0, l)
+            assert v["len"] == hb.hermes_layer_budget(h, l)
+            out.append({k: v[k].clone() for k in ("k", "v", "pos", "last_kept", "last_scores")})
+        torch.cuda.synchronize()
+        assert hb.hermes_device_status(h) == 0
+        hb.hermes_destroy(h)
+        caches.append(out)
+    for l in range(L):
+        for k in caches[0][l]:
+            assert torch.equal(caches[0][l][k], caches[1][l][k]), f"layer {l}: {k} differs between deferred and immediate V compaction"
