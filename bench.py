@@ -29,7 +29,7 @@ POOL = 16          # distinct pre-generated chunk/probe sets cycled through the 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at configs[1], transcribed from the one
 # `ncu --set full` capture summarised in profiles/r2_ncu_full_summary.txt (command in profiles/r2_README.md);
 # the scoring kernel's figure includes the previous update's V compaction (360 MB) that rides in it
-NCU_TRAFFIC_BYTES = {"gather": 181.35e6 + 132.91e6, "score": 561.52e6 + 189.66e6,
+NCU_TRAFFIC_BYTES = {"gather": 181.35e6 + 132.39e6, "score": 561.45e6 + 188.30e6,
                      "select": 1.44e6, "append": 11.25e6}
 
 
