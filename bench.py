@@ -180,6 +180,8 @@ def run_ours(args, backend=None, hb=None):
         be.init_process_group(dist)
     dev = be.dev
     wl = workload_by_name(args.workload)
+    if args.streams > 0:                                     # independent streams advanced by one call (one handle)
+        wl = wl.scaled(n_streams=args.streams)
     B = wl.n_streams
     tdt = torch.bfloat16 if wl.dtype == "bf16" else torch.float32
     over = dict(score_path={"auto": 0, "simt": 1, "tcgen05": 2}[args.score_path])
@@ -431,6 +433,7 @@ def main():
     ap.add_argument("--score-path", default="auto", choices=["auto", "simt", "tcgen05"])
     ap.add_argument("--reindex", default="eager", choices=["eager", "lazy"])
     ap.add_argument("--max-position", type=int, default=32768, help="lazy re-indexing: the model's position limit")
+    ap.add_argument("--streams", type=int, default=0, help="streams per GPU advanced by one call (0: the workload's own count)")
     ap.add_argument("--summary-token", action="store_true")
     ap.add_argument("--budget-weight", default="", help="layer-dependent budgets: shallow,middle,deep weights (PAPER.md Tab. 5), e.g. 1.3,1.0,0.7")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -168,7 +168,7 @@ def _ours_worker(rank: int, world: int, port: int, out_dir: str):
     bench.CONFIGS["llava_ov_7b"] = small
     args = argparse.Namespace(gpus=world, steps=3, warmup=3, impl="ours", workload="llava_ov_7b", score_path="auto",
                               reindex="eager", max_position=32768, summary_token=False, no_cpu_baseline=True,
-                              no_defer_v=False, no_replay_check=False, budget_weight="")
+                              no_defer_v=False, no_replay_check=False, budget_weight="", streams=0)
     fake = _FakeHermes()
     out = bench.run_ours(args, backend=_CpuBackend(), hb=fake)
     with open(os.path.join(out_dir, f"o{rank}.json"), "w") as f:
