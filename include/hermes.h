@@ -25,6 +25,11 @@
  *     hermes_workspace_bytes() bytes (256-byte aligned), which the handle owns until hermes_destroy().
  *   - Query head h uses KV head h / (n_q_heads / n_kv_heads) (grouped-query attention).
  *   - A handle is not thread-safe; use one per host thread or serialise calls.
+ *   - hermes_append_chunk() with uniform budgets enqueues kernels only (no copy, no allocation, no host synchronisation), so it
+ *     may be called on a capturing stream.  The handle's host-side state advances when the call is made, not when the graph
+ *     runs: capture in steady state (eager re-indexing, len == budget, default pos_start, fixed n_new / n_probe) and an EVEN
+ *     number of updates (the double buffer flips once per evicting update); such a graph can be replayed with new data
+ *     in the same input buffers, and hermes_get_cache() stays valid after any number of replays.
  *   - The tcgen05 scoring kernel is persistent (at most one CTA per SM) and a CTA's second pass waits for row
  *     statistics written by other CTAs of the same launch, so every CTA of its grid must be resident at once.  It is
  *     launched cooperatively: on a device partition that cannot hold the grid (MPS active-thread percentage, a green

@@ -424,3 +424,46 @@ def test_deferred_v_compaction_equals_immediate():
     # and the lock-step oracle comparison still holds when every checked update starts from a flushed cache
     ls, reps = _run(wl, 3, n_warm=2, cfg_over=dict(defer_v=1))
     ls.close()
+
+
+def test_steady_state_updates_replay_from_a_cuda_graph():
+    """An evicting update on the device entry point enqueues kernels only (no copy, no allocation, no host
+    synchronisation; cooperative + programmatic-dependent launches included), so it can be stream-captured.  In steady
+    state (eager re-indexing, len == budget, default pos_start) two consecutive updates form a period -- the double buffer
+    flips twice, every kernel argument repeats -- and a graph of two updates replayed n times equals 2 n eager updates on
+    the same input buffers, bit for bit (the V move rides inside the captured scoring launches as well)."""
+    wl = CONFIGS["llava_ov_7b"].scaled(n_layers=6, budget=784, probe_tokens=64)
+    gen = torch.Generator(device="cuda").manual_seed(11)
+    L, C = wl.n_layers, wl.chunk_tokens
+    K, V = (torch.randn(1, L, C, wl.n_kv_heads, wl.head_dim, generator=gen, device="cuda").to(torch.bfloat16) for _ in range(2))
+    Q = torch.randn(1, L, wl.n_q_heads, wl.probe_tokens, wl.head_dim, generator=gen, device="cuda").to(torch.bfloat16)
+    K2, V2, Q2 = K.clone(), V.clone(), Q.clone()              # the eager handle reads its own copies
+
+    def warm(k, v, q):
+        h = hb.hermes_create(hb.config_for_workload(wl))
+        for _ in range(wl.budget // C):
+            hb.hermes_append_chunk(h, k, v, None)
+        for _ in range(2):
+            hb.hermes_append_chunk(h, k, v, q)
+        return h
+
+    a, b = warm(K, V, Q), warm(K2, V2, Q2)
+    torch.cuda.synchronize()
+    graph, side = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+    with torch.cuda.graph(graph, stream=side):                # the binding launches on torch's current stream: the capturing one
+        hb.hermes_append_chunk(a, K, V, Q)
+        hb.hermes_append_chunk(a, K, V, Q)
+    for i in range(4):
+        fresh = torch.randn(K.shape, generator=gen, device="cuda").to(torch.bfloat16)
+        K.copy_(fresh); K2.copy_(fresh)                       # new data in the same buffers, as a serving loop would do
+        graph.replay()
+        hb.hermes_append_chunk(b, K2, V2, Q2)
+        hb.hermes_append_chunk(b, K2, V2, Q2)
+        torch.cuda.synchronize()
+    assert hb.hermes_last_score_path(a) == hb.HERMES_SCORE_TCGEN05 and hb.hermes_len(a) == hb.hermes_len(b) == wl.budget
+    for l in range(L):
+        va, vb = hb.hermes_get_cache(a, 0, l), hb.hermes_get_cache(b, 0, l)
+        torch.cuda.synchronize()
+        for k in ("k", "v", "pos", "last_kept", "last_scores"):
+            assert torch.equal(va[k], vb[k]), f"layer {l}: {k} differs between graph replay and eager updates"
+    hb.hermes_destroy(a); hb.hermes_destroy(b)
