@@ -527,10 +527,16 @@ def oracle_step_layer_budgets(st: OracleStream, K_new: np.ndarray, V_new: np.nda
     to, not re-indexed) otherwise.  Arrival positions are shared by all layers and lie above every cached position:
     1D default offset + max_l len_l.  Scores of layer l are taken over its own T_l = len_l + n_new candidates, the
     recency term counts the distance from ITS newest token, and Eq. 5 pairs candidates at equal distance from the
-    newest token (`smooth_scores_aligned`).  1D RoPE, no summary token.  With equal weights this is `oracle_step`."""
+    newest token (`smooth_scores_aligned`).  1D RoPE.  With equal weights this is `oracle_step`.
+
+    Summary tokens (Alg. 1; DESIGN f1 x f4): a DEEP layer that compresses at this arrival keeps m_l - 1 tokens by Top-K and
+    appends one summary token of everything it evicts in slot m_l - 1, exactly as in `oracle_step` with m_l for |M|: target
+    position offset + m_l - 1 at a step that re-indexes, the position after the newest token otherwise (the running
+    position counter then advances by one more -- once, whatever the number of deep layers that made one).  A deep layer
+    still under its budget makes none."""
     cfg = st.cfg
-    if cfg.rope_mode != "1d" or cfg.summary_token:
-        raise ValueError("layer-dependent budgets are defined here for 1D RoPE without summary tokens (DESIGN f4)")
+    if cfg.rope_mode != "1d":
+        raise ValueError("layer-dependent budgets are defined here for 1D RoPE (DESIGN f4)")
     L, n_new = K_new.shape[0], K_new.shape[1]
     m = layer_budgets(cfg)
     if st.lens is None:
@@ -564,12 +570,30 @@ def oracle_step_layer_budgets(st: OracleStream, K_new: np.ndarray, V_new: np.nda
         w = omega_of_layer(cfg, l)
         S.append((1.0 - w) * normalise_attention(W, cfg.norm_mode) + w * R)
     S_tilde = smooth_scores_aligned(cfg, S)
-    reindex = cfg.reindex_mode == "eager" or lazy_reindex_due(cfg, p_end)
+    summ = [bool(cfg.summary_token and layer_stage(cfg, l) == "deep" and over[l]) for l in range(L)]
+    summ_pos = 1 if any(summ) else 0
+    reindex = cfg.reindex_mode == "eager" or lazy_reindex_due(cfg, p_end + summ_pos)
     kept, pos_new = [], []
     new_lens = T.copy()
     for l in range(L):
         if not over[l]:                                   # under its budget: nothing happens to this layer
             kept.append(np.arange(T[l])); pos_new.append(st.pos[l][:, :T[l]].copy())
+            continue
+        if summ[l]:
+            n_keep = int(m[l]) - 1
+            I = select_topk(S_tilde[l], n_keep)
+            ev = np.setdiff1d(np.arange(T[l]), I)
+            p_old = st.pos[l][:, I]
+            p_new = compact_positions(cfg, p_old) if reindex else p_old
+            t = cfg.pos_offset + n_keep if reindex else p_end
+            k_sum, v_sum = summary_token(cfg, st.K[l, ev], st.V[l, ev], st.pos[l][:, ev], t)
+            V_kept = st.V[l, I].copy()
+            K_kept = rotary_delta(cfg, st.K[l, I], p_new - p_old)
+            st.V[l, :n_keep], st.V[l, n_keep] = V_kept, v_sum
+            st.K[l, :n_keep], st.K[l, n_keep] = K_kept, k_sum
+            st.pos[l, :, :n_keep], st.pos[l, :, n_keep] = p_new, t
+            kept.append(np.concatenate([I, [-1]])); pos_new.append(st.pos[l][:, :m[l]].copy())
+            new_lens[l] = m[l]
             continue
         I = select_topk(S_tilde[l], int(m[l]))
         p_old = st.pos[l][:, I]
@@ -583,6 +607,8 @@ def oracle_step_layer_budgets(st: OracleStream, K_new: np.ndarray, V_new: np.nda
     st.len = int(new_lens.max())
     if reindex:                                           # positions of the layers that compressed are below offset + m_l
         st.next_pos = max(cfg.pos_offset + int(new_lens.max()), p_end if (~over).any() else 0)
+    else:
+        st.next_pos = p_end + summ_pos
     st.last = {"T": T.copy(), "evicted": True, "evicted_layers": over.copy(), "reindexed": reindex, "S": S,
                "S_tilde": S_tilde, "kept": kept, "pos_new": pos_new, "budgets": m}
     return st.last

@@ -2,7 +2,7 @@
 import numpy as np
 import pytest
 
-from helpers import Feeder, oracle_config, run_oracle_schedule
+from helpers import Feeder, oracle_config, run_oracle_schedule, take_ids
 from oracle import hermes_oracle as ho
 from workloads import CONFIGS, rope_at_arrival
 
@@ -72,8 +72,8 @@ def _run_lb(wl, n_updates, w, **over):
         for l in range(L):
             ids[l] = np.concatenate([ids[l], new_ids])
             if out["evicted"]:
-                ids[l] = ids[l][out["kept"][l]]
-        hist.append(dict(out=out, pre=pre, K_new=K, V_new=V))
+                ids[l] = take_ids(ids[l][None, :], np.asarray(out["kept"][l])[None, :])[0]   # -1: a summary token
+        hist.append(dict(out=out, pre=pre, K_new=K, V_new=V, p_arr=ap))
     return cfg, st, fd, ids, hist
 
 
@@ -128,3 +128,60 @@ def test_pure_recency_layers_keep_their_newest_m_l_tokens():
     m = ho.layer_budgets(cfg)
     for l in range(wl.n_layers):                                # sliding window of PAPER.md:49, one width per layer
         assert ids[l].tolist() == list(range(fd.tokens_fed - m[l], fd.tokens_fed))
+
+
+# ---- summary tokens under layer-dependent budgets (DESIGN f1 x f4) ---------------------------------------------
+def test_equal_weights_with_summary_token_reproduce_the_uniform_path_bit_for_bit():
+    wl = CONFIGS["toy"]
+    _, st_u, _, ids_u, hist_u = run_oracle_schedule(wl, 6, cfg_over=dict(summary_token=True))
+    cfg, st, fd, ids, hist = _run_lb(wl, 6, (1.0, 1.0, 1.0), capacity=wl.cap, summary_token=True)
+    M = wl.budget
+    assert (st.lens == M).all() and st.next_pos == st_u.next_pos
+    assert st.K[:, :M].tobytes() == st_u.K[:, :M].tobytes() and st.V[:, :M].tobytes() == st_u.V[:, :M].tobytes()
+    assert np.array_equal(st.pos[:, :, :M], st_u.pos[:, :, :M]) and np.array_equal(np.stack(ids), ids_u)
+
+
+@pytest.mark.parametrize("lazy", [False, True])
+@pytest.mark.parametrize("w", TAB5[1:])
+def test_summary_token_of_a_deep_layer_is_alg1_of_what_that_layer_evicted(w, lazy):
+    """Toy: 4 layers, layer 3 deep.  At every step at which layer 3 compresses, its last slot (m_3 - 1) is Alg. 1 recomputed
+    here from the candidates it evicted (previous cache + chunk, at their positions); the other layers never hold one; a
+    step at which layer 3 is still under its budget makes none.  Lazy mode: target = the position after the newest token,
+    and the next chunk starts one position later."""
+    wl = CONFIGS["toy"]
+    over = dict(summary_token=True)
+    if lazy:
+        over.update(reindex_mode="lazy", max_position=100000, max_chunk_span=wl.chunk_tokens)
+    cfg, st, fd, ids, hist = _run_lb(wl, 8, w, **over)
+    m = ho.layer_budgets(cfg)
+    made = 0
+    for h in hist[1:]:
+        out, pre = h["out"], h["pre"]
+        n3, n_new = int(pre["lens"][3]), h["K_new"].shape[1]
+        T3 = n3 + n_new
+        if not out["evicted"] or T3 <= m[3]:
+            if out["evicted"]:
+                assert np.array_equal(out["kept"][3], np.arange(T3))        # untouched: no summary token
+            continue
+        kept3 = np.asarray(out["kept"][3])
+        assert len(kept3) == m[3] and kept3[-1] == -1 and (np.diff(kept3[:-1]) > 0).all()
+        for l in range(3):
+            assert (np.asarray(out["kept"][l]) >= 0).all()
+        K_cand = np.concatenate([pre["K"][3, :n3], h["K_new"][3]], axis=0)
+        V_cand = np.concatenate([pre["V"][3, :n3], h["V_new"][3]], axis=0)
+        P_cand = np.concatenate([pre["pos"][3][:, :n3], h["p_arr"]], axis=1)
+        ev = np.setdiff1d(np.arange(T3), kept3[:-1])
+        assert len(ev) == T3 - (m[3] - 1)
+        p_end = int(h["p_arr"][0, -1]) + 1
+        t = cfg.pos_offset + m[3] - 1 if out["reindexed"] else p_end
+        k_sum, v_sum = ho.summary_token(cfg, K_cand[ev], V_cand[ev], P_cand[:, ev], t)
+        assert out["pos_new"][3][0, -1] == t and (np.diff(out["pos_new"][3][0]) > 0).all()
+        made += 1
+        h["expect"] = (k_sum, v_sum)
+    assert made >= 5
+    # the last step's summary token is still in the cache as computed
+    k_sum, v_sum = hist[-1]["expect"]
+    assert np.array_equal(st.K[3, m[3] - 1], k_sum) and np.array_equal(st.V[3, m[3] - 1], v_sum)
+    assert ids[3][-1] == -1 and all((i >= 0).all() for i in ids[:3])
+    if lazy:                                                                # one position per step went to a summary token
+        assert st.next_pos == cfg.pos_offset + fd.tokens_fed + made
