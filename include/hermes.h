@@ -103,8 +103,8 @@ typedef struct {
   float budget_weight[3];       /* layer-dependent budgets (Tab. 5): weight of a shallow / middle / deep
                                    layer.  With the total budget * n_layers fixed, layer i keeps
                                    m_i = floor(w_i / sum_j w_j * budget * n_layers) tokens, the residue goes to the last
-                                   layer.  {1, 1, 1} (default): `budget` everywhere.  Unequal weights need HERMES_ROPE_1D
-                                   and no summary token                                                           */
+                                   layer.  {1, 1, 1} (default): `budget` everywhere.  Unequal weights need HERMES_ROPE_1D;
+                                   with summary_token a deep layer i keeps m_i - 1 tokens + its summary token     */
   int32_t defer_v;              /* 1 (default): on the tcgen05 path an eviction compacts K at once but leaves the
                                    kept V rows to be moved by the NEXT update's scoring kernel (V is not read by
                                    scoring, so the copy hides behind it); hermes_get_cache() and updates that do

@@ -107,7 +107,7 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
     if (fa.sharedSizeBytes + size_t(y.cap) * 4 > prop.sharedMemPerBlockOptin)
       return fail(nullptr, HERMES_EINVAL, "max_tokens %d too large for the select kernel's shared memory", y.cap);
     if (c->summary_token) {
-      const size_t need = size_t(y.cap - c->budget + 2) * 8;
+      const size_t need = size_t(y.cap - y.budget_min + 2) * 8;
       cudaFuncAttributes fs;
       CUDA_TRY(nullptr, c->dtype == HERMES_BF16 ? cudaFuncGetAttributes(&fs, k_summary<__nv_bfloat16>) : cudaFuncGetAttributes(&fs, k_summary<float>));
       if (fs.sharedSizeBytes + need > prop.sharedMemPerBlockOptin)
@@ -136,7 +136,7 @@ extern "C" int hermes_create(const hermes_config* c, void* workspace, size_t byt
   g.cap = y.cap; g.budget = y.budget_max; g.n_axes = y.n_axes; g.row_elems = c->n_kv_heads * c->head_dim;
   g.lay_T = h->lb ? reinterpret_cast<const int32_t*>(h->ws + y.lay_dyn) : nullptr;
   g.lay_keep = h->lb ? g.lay_T + c->n_layers : nullptr;
-  g.n_shallow = y.n_shallow; g.n_deep = y.n_deep; g.summary = c->summary_token; g.probe_deep_begin = c->probe_deep_begin; g.n_evict_max = y.cap - c->budget + 1;
+  g.n_shallow = y.n_shallow; g.n_deep = y.n_deep; g.summary = c->summary_token; g.probe_deep_begin = c->probe_deep_begin; g.n_evict_max = y.cap - y.budget_min + 1;
   g.p_max = c->max_probe_tokens; g.pos_offset = c->pos_offset;
   g.sec_t = c->mrope_section[0]; g.sec_h = c->mrope_section[1];
   g.compact_axes = c->mrope_compact_axes; g.grid_h = c->mrope_grid_h; g.grid_w = c->mrope_grid_w;
@@ -410,7 +410,13 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
   const long long span_max = g.n_axes == 1 ? c.max_chunk_tokens
                                            : (c.max_chunk_tokens + c.mrope_grid_h * c.mrope_grid_w - 1) / (c.mrope_grid_h * c.mrope_grid_w);
   // a summary token takes the position after the newest token (DESIGN f1): the running counter advances by one more
-  const int summ_pos = (c.summary_token && h->lay.n_deep > 0) ? 1 : 0;
+  int summ_pos = (c.summary_token && h->lay.n_deep > 0) ? 1 : 0;
+  int n_ev_max = Tn - c.budget + 1;                  // longest evicted list a summary token is made of
+  if (h->lb && summ_pos) {                           // layer-dependent budgets: only if a deep layer compresses at this arrival
+    summ_pos = 0; n_ev_max = 0;
+    for (int l = c.n_layers - h->lay.n_deep; l < c.n_layers; ++l)
+      if (dyn[c.n_layers + l] < dyn[l]) { summ_pos = 1; n_ev_max = std::max(n_ev_max, int(dyn[l] - dyn[c.n_layers + l] + 1)); }
+  }
   const bool reindex = !lazy || p0 + span + summ_pos + span_max > c.max_position;
   if (lazy && p0 + span > c.max_position) return fail(h, HERMES_ECAPACITY, "positions would exceed max_position %d", c.max_position);
 
@@ -497,13 +503,13 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
       launch_pdl(k_select, dim3(BL), dim3(kSelThreads), size_t(Tn) * 4, s, g, h->cur, Tn, c.forget_rate, int(c.norm_mode == HERMES_NORM_SUM), r_norm_sum, int(reindex),
                  reindex ? c.pos_offset + c.budget - 1 : int(p0 + span));
     }
-    if (c.summary_token && h->lay.n_deep > 0) {
+    if (summ_pos) {
       Prof p(h, HERMES_K_SUMMARY, s);
       const dim3 sgrid(g.Hkv, g.B * h->lay.n_deep), sblock(64 * kSumLanes);
-      const size_t ssm = size_t(Tn - c.budget + 1) * 8;
-      const int st_pos = reindex ? c.pos_offset + c.budget - 1 : int(p0 + span);
-      const cudaError_t es = c.dtype == HERMES_BF16 ? launch_pdl(k_summary<__nv_bfloat16>, sgrid, sblock, ssm, s, g, h->cur, Tn, st_pos)
-                                                    : launch_pdl(k_summary<float>, sgrid, sblock, ssm, s, g, h->cur, Tn, st_pos);
+      const size_t ssm = size_t(n_ev_max) * 8;
+      const int st_pos = int(p0 + span);                 // target between re-index steps; at one: offset + m_l - 1, per layer
+      const cudaError_t es = c.dtype == HERMES_BF16 ? launch_pdl(k_summary<__nv_bfloat16>, sgrid, sblock, ssm, s, g, h->cur, Tn, st_pos, int(reindex))
+                                                    : launch_pdl(k_summary<float>, sgrid, sblock, ssm, s, g, h->cur, Tn, st_pos, int(reindex));
       if (es != cudaSuccess) return fail(h, HERMES_ECUDA, "summary kernel launch: %s", cudaGetErrorString(es));
     }
     {
@@ -531,7 +537,7 @@ static int append_impl(hermes_t* h, const void* K_new, const void* V_new, const 
     if (evict) { h->cur ^= 1; h->last_T = Tn; }
     h->len = mx;
     // after a re-index step every position of a layer that compressed is below offset + m_l (DESIGN f4)
-    h->next_pos = (!evict || !reindex) ? p0 + n_new : std::max<long long>(c.pos_offset + mx, untouched ? p0 + n_new : 0);
+    h->next_pos = (!evict || !reindex) ? p0 + n_new + (evict ? summ_pos : 0) : std::max<long long>(c.pos_offset + mx, untouched ? p0 + n_new : 0);
   } else if (evict) {
     h->cur ^= 1; h->len = c.budget; h->last_T = Tn;
     if (!reindex) h->next_pos = p0 + span + summ_pos; else

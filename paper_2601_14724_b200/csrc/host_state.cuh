@@ -97,9 +97,9 @@ inline const char* validate(const hermes_config& c) {
   if (c.score_path < HERMES_SCORE_AUTO || c.score_path > HERMES_SCORE_TCGEN05) return "bad score_path";
   for (float w : c.budget_weight) if (!(w > 0.f) || !std::isfinite(w)) return "budget_weight must be positive";
   if (!uniform_budgets(c)) {
-    if (c.rope_mode != HERMES_ROPE_1D || c.summary_token) return "layer-dependent budgets need 1D RoPE and no summary token";
+    if (c.rope_mode != HERMES_ROPE_1D) return "layer-dependent budgets need 1D RoPE";
     for (int m : layer_budgets(c, ns, nd)) {
-      if (m < 1) return "a layer's budget would be zero";
+      if (m < (c.summary_token ? 2 : 1)) return "a layer's budget would be zero (or, with summary tokens, below 2)";
       if (c.max_tokens != 0 && c.max_tokens <= m) return "max_tokens must exceed the largest layer budget (or be 0)";
     }
   }
@@ -143,14 +143,14 @@ inline Layout make_layout(const hermes_config& c) {
   y.scores = take(BL * y.cap * 4);
   y.kept = take(BL * y.budget_max * 4);
   y.delta = take(BL * y.n_axes * y.budget_max * 4);
-  y.evicted = take(BL * size_t(y.cap - c.budget + 1) * 4);
+  y.evicted = take(BL * size_t(y.cap - y.budget_min + 1) * 4);
   y.rope_tab = take(size_t(y.table_rows) * (c.head_dim / 2) * 8);
   y.rope_freq = take(size_t(c.head_dim / 2) * 8);
   // summary tokens: (cos, sin)(delta * theta_j) for delta in [-sum_tab_neg, sum_tab_rows - sum_tab_neg).  Eager: an evicted
   // token moves from p in [offset, offset + cap) to t = offset + budget - 1.  Lazy: to the position after the newest token
   // (delta up to max_position - offset), and back down at a re-index step.  Capped at 2 x 65536 rows; beyond: fp64 sincos.
-  y.sum_tab_neg = y.cap - c.budget + 1;
-  int sum_pos = c.budget + 1;
+  y.sum_tab_neg = y.cap - y.budget_min + 1;
+  int sum_pos = y.budget_max + 1;
   if (c.reindex_mode == HERMES_REINDEX_LAZY) {
     y.sum_tab_neg = std::min(65536, std::max(y.sum_tab_neg, c.max_position - c.pos_offset + 1));
     sum_pos = std::min(65536, std::max(sum_pos, c.max_position - c.pos_offset + 1));

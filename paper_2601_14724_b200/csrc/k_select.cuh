@@ -181,7 +181,7 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
   // deep layers of a summary-token cache keep one token fewer: slot budget-1 is the summary token (DESIGN f1)
   const bool summ = g.summary && l >= g.L - g.n_deep;
   const int n_keep = budget_l - (summ ? 1 : 0);
-  if (n_keep >= Tn) {
+  if (budget_l >= Tn) {
     // layer-dependent budgets: this layer is under its budget at this arrival -- nothing is evicted, nothing re-indexed
     // (1D RoPE only, validated at create); the gather then copies every row as it is
     const int32_t* po = g.posc + (size_t(bl) * 2 + cur) * g.n_axes * g.cap;
@@ -315,7 +315,7 @@ k_select(Geom g, int cur, int Tn, float k_forget, int norm_sum, float r_norm_sum
     }
   }
   if (summ && tid == 0) {                               // the summary token's slot (filled by k_summary)
-    kept[n_keep] = -1; pos_new[n_keep] = summary_pos; dl1[n_keep] = 0;
+    kept[n_keep] = -1; pos_new[n_keep] = reindex ? g.pos_offset + n_keep : summary_pos; dl1[n_keep] = 0;
   }
   if (g.n_axes == 1) return;
   __syncthreads();                                      // kept[] visible to the whole block

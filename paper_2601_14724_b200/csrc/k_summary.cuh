@@ -15,7 +15,7 @@ constexpr int kSumLanes = 16;
 
 template <typename T>
 __global__ void __launch_bounds__(64 * kSumLanes)
-k_summary(Geom g, int cur, int Tn, int t) {
+k_summary(Geom g, int cur, int Tn, int t, int reindex) {
   __shared__ double red[kSumLanes][4][64];                 // [token lane][kx, ky, vx, vy][pair]
   extern __shared__ int s_list[];                          // [2][n_ev]: source row, rotary delta of every evicted token
   pdl_wait();
@@ -25,7 +25,12 @@ k_summary(Geom g, int cur, int Tn, int t) {
   const int kvh = blockIdx.x;
   const int b = blockIdx.y / g.n_deep, l = g.L - g.n_deep + blockIdx.y % g.n_deep;
   const int bl = b * g.L + l;
-  const int n_keep = g.budget - 1, n_ev = Tn - n_keep;
+  // layer-dependent budgets (DESIGN f1 x f4): this layer's own candidates and budget; a layer still under its budget at this
+  // arrival evicts nothing and makes no summary token
+  Tn = layer_T(g, l, Tn);
+  if (layer_keep(g, l) >= Tn) return;
+  const int n_keep = layer_keep(g, l) - 1, n_ev = Tn - n_keep;
+  if (reindex) t = g.pos_offset + n_keep;               // the next contiguous position (Alg. 1 step 3)
   const size_t slab_src = size_t(bl) * 2 + cur, slab_dst = size_t(bl) * 2 + (cur ^ 1);
   const T* ks = reinterpret_cast<const T*>(g.kc) + slab_src * g.cap * g.row_elems + kvh * g.d;
   const T* vs = reinterpret_cast<const T*>(g.vc) + slab_src * g.cap * g.row_elems + kvh * g.d;

@@ -94,9 +94,10 @@ def test_layer_dependent_budget_configs():
     assert hb.hermes_workspace_bytes(hb.config_for_workload(wl, budget_weight=(1.3, 1.0, 0.7))) == 0   # max_tokens < largest layer
     ok = hb.config_for_workload(wl, budget_weight=(1.3, 1.0, 0.7), max_tokens=0)
     assert hb.hermes_workspace_bytes(ok) > hb.hermes_workspace_bytes(hb.config_for_workload(wl))   # slabs sized for the largest layer
-    for bad in (dict(budget_weight=(1.3, 1.0, 0.0)), dict(budget_weight=(1.3, 1.0, 0.7), summary_token=1),
+    for bad in (dict(budget_weight=(1.3, 1.0, 0.0)),
                 dict(budget_weight=(0.7, 1.0, 1.3), rope_mode=hb.HERMES_ROPE_M3D)):
         assert hb.hermes_workspace_bytes(hb.config_for_workload(wl, max_tokens=0, **bad)) == 0
+    assert hb.hermes_workspace_bytes(hb.config_for_workload(wl, max_tokens=0, budget_weight=(1.3, 1.0, 0.7), summary_token=1)) > 0
     # both scoring paths take per-layer candidate counts
     assert hb.hermes_workspace_bytes(hb.config_for_workload(wl, max_tokens=0, budget_weight=(1.3, 1.0, 0.7), score_path=hb.HERMES_SCORE_TCGEN05)) > 0
 

@@ -31,8 +31,8 @@ def _gpu_state(h, ocfg, wl):
     return st
 
 
-def _run(wl, w, n_updates, **over):
-    ocfg = oracle_config(wl, budget_weights=w, capacity=0)
+def _run(wl, w, n_updates, oover=None, **over):
+    ocfg = oracle_config(wl, budget_weights=w, capacity=0, **(oover or {}))
     m = ho.layer_budgets(ocfg)
     # slots per layer: the largest layer plus a chunk, and at least the workload's own capacity (the toy preload)
     cfg = hb.config_for_workload(wl, budget_weight=w, max_tokens=int(max(wl.cap, m.max() + wl.chunk_tokens)), **over)
@@ -42,14 +42,18 @@ def _run(wl, w, n_updates, **over):
     half = wl.head_dim // 2
     n_cmp = n_untouched = 0
     paths = set()
+    n_summ = 0
     sizes = [wl.preload_tokens] if wl.preload_tokens else []
+    next_pos = -1                                           # lazy mode: the running position counter, mirrored from the oracle
     for u, n in enumerate(sizes + [wl.chunk_tokens] * n_updates):
         st = _gpu_state(h, ocfg, wl)
+        st.next_pos = next_pos
         ap = ho.arrival_positions(ocfg, st, n, -1)
         K, V, Q, _ = fd.next(n, ap, with_probe=u >= len(sizes))
         hb.hermes_append_chunk(h, to_dev(K[None], wl.dtype), to_dev(V[None], wl.dtype), None if Q is None else to_dev(Q[None], wl.dtype))
         torch.cuda.synchronize()
         out = ho.oracle_step_layer_budgets(st, K, V, Q)
+        next_pos = st.next_pos
         if out["evicted"]:
             paths.add(hb.hermes_last_score_path(h))
         assert hb.hermes_len(h) == int(st.lens.max())
@@ -69,8 +73,18 @@ def _run(wl, w, n_updates, **over):
             rel = np.abs(s_gpu - s_or) / np.maximum(np.abs(s_or), 1e-30)
             assert (rel <= SCORE_RTOL).all(), f"layer {l}: score rel err {rel.max():.3e}"
             kept_gpu = v["last_kept"].cpu().numpy().astype(np.int64)
-            kept_or = out["kept"][l]
-            assert len(kept_gpu) == m[l] and (np.diff(kept_gpu) > 0).all()
+            kept_or = np.asarray(out["kept"][l])
+            assert len(kept_gpu) == m[l]
+            if kept_or[-1] < 0:
+                # summary token (DESIGN f1 x f4) in the layer's last slot: computed values, so K AND V get the K tolerance
+                assert kept_gpu[-1] == -1 and p_gpu[0, -1] == st.pos[l, 0, n_l - 1]
+                for g_, o_ in ((k_gpu[-1], st.K[l, n_l - 1]), (v_gpu[-1], st.V[l, n_l - 1])):
+                    tol = np.maximum(K_RTOL * np.abs(o_), 2 * bf16_ulp(o_) if wl.dtype == "bf16" else 0.0) + 1e-30
+                    assert (np.abs(g_.astype(np.float64) - o_) <= tol).all(), f"layer {l}: summary token off"
+                n_summ += 1
+                kept_gpu, kept_or = kept_gpu[:-1], kept_or[:-1]
+                k_gpu, v_gpu, p_gpu, n_l = k_gpu[:-1], v_gpu[:-1], p_gpu[:, :-1], n_l - 1
+            assert (np.diff(kept_gpu) > 0).all() and kept_gpu[0] >= 0
             if not np.array_equal(kept_gpu, kept_or):
                 tau = s_or[kept_or].min()
                 diff = np.setxor1d(kept_gpu, kept_or)
@@ -88,6 +102,7 @@ def _run(wl, w, n_updates, **over):
     assert hb.hermes_device_status(h) == 0 and hb.hermes_v_pending(h) == 0
     lens = [hb.hermes_layer_len(h, l) for l in range(wl.n_layers)]
     hb.hermes_destroy(h)
+    _run.n_summ = n_summ
     return m, lens, n_cmp, n_untouched, paths
 
 
@@ -163,3 +178,24 @@ def test_deferred_v_move_with_layer_budgets_full_size():
     for l in range(L):
         for k in caches[0][l]:
             assert torch.equal(caches[0][l][k], caches[1][l][k]), f"layer {l}: {k} differs between deferred and immediate V compaction"
+
+
+@pytest.mark.parametrize("lazy", [False, True])
+@pytest.mark.parametrize("w", TAB5)
+def test_summary_token_with_layer_budgets_toy(w, lazy):
+    """DESIGN f1 x f4: a deep layer that compresses keeps m_l - 1 tokens and one summary token of what it evicted; eager and
+    lazy re-indexing (lazy: the running position advances by one more at such a step)."""
+    wl = CONFIGS["toy"]
+    over, oover = dict(summary_token=1), dict(summary_token=True)
+    if lazy:
+        over.update(reindex_mode=hb.HERMES_REINDEX_LAZY, max_position=420)       # re-index steps inside the run
+        oover.update(reindex_mode="lazy", max_position=420, max_chunk_span=wl.chunk_tokens)
+    m, lens, n_cmp, _, paths = _run(wl, w, 8, oover=oover, **over)
+    assert lens == m.tolist() and n_cmp >= 18 and _run.n_summ >= 5
+
+
+def test_summary_token_with_layer_budgets_on_tcgen05():
+    wl = CONFIGS["llava_ov_7b"].scaled(n_layers=7, budget=896, probe_tokens=24)    # 1 / 4 / 2 layers: two deep layers
+    m, lens, n_cmp, _, paths = _run(wl, (1.3, 1.0, 0.7), 9, oover=dict(summary_token=True), summary_token=1,
+                                    score_path=hb.HERMES_SCORE_TCGEN05)
+    assert lens == np.minimum(m, 196 * 9).tolist() and paths == {hb.HERMES_SCORE_TCGEN05} and _run.n_summ >= 8
