@@ -18,7 +18,7 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {           // byte offsets into the workspace
   size_t kc, vc, posc, colsum, wsum, wmax, rowstat, partial, scores, kept, delta, evicted, rope_tab, rope_freq, sum_tab, omega, lambda,
-      status, seg_cnt, lay_dyn, stage_k, stage_v, stage_q, tmaps, total;
+      status, seg_cnt, lay_dyn, tc_pre, stage_k, stage_v, stage_q, tmaps, total;
   int cap, n_axes, n_part_max, table_rows, n_shallow, n_middle, n_deep, n_vh_max, sum_tab_neg, sum_tab_rows;
   int budget_max, budget_min;   // largest / smallest layer budget (= budget unless budget_weight is unequal)
   size_t esize, row_bytes, stage_kv_bytes, stage_q_bytes;
@@ -162,6 +162,7 @@ inline Layout make_layout(const hermes_config& c) {
   y.status = take(256);
   y.seg_cnt = take(BL * y.n_vh_max * 4);
   y.lay_dyn = take(size_t(c.n_layers) * 2 * 4);
+  y.tc_pre = take((BL + 1) * 2 * 4);              // layer-dependent budgets on the tcgen05 path: segment / tile prefix sums
   // staging of the host entry point, two sets: the copies of call n + 1 run while the kernels of call n read set n & 1
   y.stage_kv_bytes = align_up(BL * c.max_chunk_tokens * y.row_bytes);
   y.stage_q_bytes = align_up(BL * rows * c.head_dim * y.esize);

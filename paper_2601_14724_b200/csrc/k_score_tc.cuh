@@ -54,6 +54,11 @@ struct TcArgs {
   int v_src_buf, v_row_bytes;
   int v_n_new;              // layer-dependent budgets: rows layer l held after the previous update = lay_T[l] - v_n_new
   int v_ring_bytes;         // staging ring of the mover: a whole number of rows (tc_ring_bytes)
+  // layer-dependent budgets (k_tc_score<true>): every scored layer has its own tile / segment count; pre_s / pre_t are the
+  // prefix sums of segments / tiles over the (stream, scored layer) blocks of Hkv * n_sc groups, [B * Ls + 1] each
+  const int32_t* pre_s;
+  const int32_t* pre_t;
+  int U1, U2;               // schedule units of pass 1 (segments) and of pass 2 (tiles)
 };
 
 // ---- schedule: CTA c owns flattened units [c*U/nC, (c+1)*U/nC) -----------------------------------
@@ -76,6 +81,26 @@ struct TcCursor {
   __device__ inline int rs_valid(const TcArgs& a) const { return min(a.RS, a.R - sc * a.RS); }
   __device__ inline int stat_row0(const TcArgs& a) const { return kvh * a.R + sc * a.RS; }
 };
+
+// Tiles / segments of a group: the launch's, or (kLb) those of its layer's own candidate count T_l.
+template <bool kLb> __device__ __forceinline__ int tc_tiles_of(const TcArgs& a, int T_l) { return kLb ? (T_l + kTcTile - 1) / kTcTile : a.tpg; }
+template <bool kLb> __device__ __forceinline__ int tc_segs_of(const TcArgs& a, int T_l) {
+  return kLb ? (tc_tiles_of<true>(a, T_l) + kTcSegTiles - 1) / kTcSegTiles : a.spg;
+}
+template <bool kLb> __device__ __forceinline__ int tc_layer_T(const TcArgs& a, const TcCursor& g) {
+  return kLb ? layer_T(a.g, a.g.n_shallow + g.ls, a.Tn) : a.Tn;
+}
+// Schedule unit u -> (group, unit inside the group).  kSeg: units are pass-1 segments, else pass-2 tiles.
+template <bool kLb, bool kSeg>
+__device__ inline void tc_locate(const TcArgs& a, int u, int& gi, int& x) {
+  if (!kLb) { const int upg = kSeg ? a.spg : a.tpg; gi = u / upg; x = u - gi * upg; return; }
+  const int32_t* pre = kSeg ? a.pre_s : a.pre_t;
+  int lo = 0, hi = a.g.B * (a.g.L - a.g.n_shallow);        // pre[lo] <= u < pre[hi] (u == total: the empty range at the end)
+  while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (__ldg(pre + mid) <= u) lo = mid; else hi = mid; }
+  const int ngb = a.g.Hkv * a.n_sc, base = __ldg(pre + lo), upg = (__ldg(pre + lo + 1) - base) / ngb;
+  const int gb = (u - base) / upg;
+  gi = lo * ngb + gb; x = u - base - gb * upg;
+}
 
 struct TcSmem {
   uint8_t* q;        // [2 halves][q_half_bytes / 128 rows][128 B], 128B-swizzled
@@ -147,16 +172,18 @@ struct TcRole { int ks = 0, kph = 0, as = 0, aph = 0, n_q = 0; };
 // Q rows of each group the CTA touches (both 64-column halves, 64-row boxes).  kSeg: unit = (group,
 // segment of kTcSegTiles tiles); otherwise unit = (group, tile).  A new group's first K tile is requested
 // before the Q buffer is waited for, so it is in flight while the old group's MMAs drain.
-template <bool kSeg>
+template <bool kSeg, bool kLb>
 __device__ inline void tc_producer(const TcSmem& s, const TcBars& b, const CUtensorMap* tq, const CUtensorMap* tk,
                                    const TcArgs& a, int u0, int u1, TcRole& st) {
-  const int upg = kSeg ? a.spg : a.tpg;
   int ks = st.ks, kph = st.kph, n_q = st.n_q;
   bool new_group = true;
-  int x = u0 % upg;
-  TcCursor g; g.init(a, u0 / upg);
+  int x, gi0;
+  tc_locate<kLb, kSeg>(a, u0, gi0, x);
+  TcCursor g; g.init(a, gi0);
+  int T_l = tc_layer_T<kLb>(a, g);
   for (int u = u0; u < u1; ++u) {
-    const int t0 = kSeg ? x * kTcSegTiles : x, t1 = kSeg ? min(a.tpg, t0 + kTcSegTiles) : x + 1;
+    const int upg = kSeg ? tc_segs_of<kLb>(a, T_l) : tc_tiles_of<kLb>(a, T_l);
+    const int t0 = kSeg ? x * kTcSegTiles : x, t1 = kSeg ? min(tc_tiles_of<kLb>(a, T_l), t0 + kTcSegTiles) : x + 1;
     const int bl = g.bl(a);
     for (int t = t0; t < t1; ++t) {
       ptx::mbar_wait(&b.k_empty[ks], kph ^ 1);
@@ -177,7 +204,7 @@ __device__ inline void tc_producer(const TcSmem& s, const TcBars& b, const CUten
         ++n_q; new_group = false;
       }
     }
-    if (++x == upg) { x = 0; g.next(a); new_group = true; }
+    if (++x == upg) { x = 0; g.next(a); new_group = true; if (kLb) T_l = tc_layer_T<true>(a, g); }
   }
   st.ks = ks; st.kph = kph; st.n_q = n_q;
 }
@@ -192,11 +219,11 @@ template <bool kEpi, bool kLb>
 __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const CUtensorMap* tmap_q, const CUtensorMap* tmap_k,
                                          const TcArgs& a, uint32_t tmem_base, TcRole& st) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int U = a.n_groups * a.spg;                                      // schedule unit = (group, segment)
+  const int U = a.U1;                                                    // schedule unit = (group, segment)
   const int s0 = tc_unit_begin(U, gridDim.x, blockIdx.x), s1 = tc_unit_begin(U, gridDim.x, blockIdx.x + 1);
 
   if (!kEpi && warp == 0) {
-    if (lane == 0) tc_producer<true>(s, b, tmap_q, tmap_k, a, s0, s1, st);
+    if (lane == 0) tc_producer<true, kLb>(s, b, tmap_q, tmap_k, a, s0, s1, st);
   } else if (!kEpi && warp == 1) {
     // ---------------- MMA issuer: the whole warp runs the loop, one elected lane issues ----------------
     const uint32_t idesc = ptx::idesc_bf16_f32(128, kTcTile);
@@ -204,14 +231,16 @@ __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const
     const uint32_t q_half16 = uint32_t(a.q_half_bytes) >> 4;
     int ks = st.ks, kph = st.kph, as = st.as, aph = st.aph, n_q = st.n_q;
     bool new_group = true;
-    int x = s0 % a.spg;
-    TcCursor g; g.init(a, s0 / a.spg);
+    int x, gi0;
+    tc_locate<kLb, true>(a, s0, gi0, x);
+    TcCursor g; g.init(a, gi0);
+    int T_l = tc_layer_T<kLb>(a, g);
     for (int u = s0; u < s1; ++u) {
       const int n_rb = (g.rs_valid(a) + 127) >> 7;
       const bool shift = g.rs_valid(a) > 384 && g.rs_valid(a) <= 448;
       if (new_group) { ptx::mbar_wait(b.q_full, n_q & 1); ++n_q; new_group = false; }
-      const bool last_seg_of_group = (u + 1 == s1) || x + 1 == a.spg;
-      const int t_end = min(a.tpg, (x + 1) * kTcSegTiles);
+      const bool last_seg_of_group = (u + 1 == s1) || x + 1 == tc_segs_of<kLb>(a, T_l);
+      const int t_end = min(tc_tiles_of<kLb>(a, T_l), (x + 1) * kTcSegTiles);
       for (int t = x * kTcSegTiles; t < t_end; ++t) {
         ptx::mbar_wait(&b.k_full[ks], kph);
         const uint32_t kb_lo = k_lo + uint32_t(ks) * (kTcKStage >> 4);
@@ -247,7 +276,7 @@ __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const
         __syncwarp();
         if (++ks == a.n_kst) { ks = 0; kph ^= 1; }
       }
-      if (++x == a.spg) { x = 0; g.next(a); new_group = true; }
+      if (++x == tc_segs_of<kLb>(a, T_l)) { x = 0; g.next(a); new_group = true; if (kLb) T_l = tc_layer_T<true>(a, g); }
     }
     st.ks = ks; st.kph = kph; st.as = as; st.aph = aph; st.n_q = n_q;
   } else if (kEpi) {
@@ -280,13 +309,13 @@ __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const
       z_run = z_run * fast_exp2(m_run - m_new) + ((sm[0] + sm[1]) + (sm[2] + sm[3]));
       m_run = m_new;
     };
-    int x = s0 % a.spg, gi = s0 / a.spg, n_done = 0;
+    int x, gi, n_done = 0;
+    tc_locate<kLb, true>(a, s0, gi, x);
     TcCursor g; g.init(a, gi);
-    // candidates of the group's layer: a.Tn, or (kLb) this layer's own count under layer-dependent budgets (DESIGN f4): the
-    // tile grid is the largest scored layer's, tokens past T_l are masked like the ragged tail of the last tile.  A template
-    // flag, not a run-time test: one more live register in this loop spills (+2 us at configs[1])
-    int T_l = a.Tn;
-    if (kLb) T_l = layer_T(a.g, g.bl(a) % a.g.L, a.Tn);
+    // candidates of the group's layer: a.Tn, or (kLb) this layer's own count under layer-dependent budgets (DESIGN f4), which
+    // also sets its tile and segment counts.  A template flag, not a run-time test: one more live register in this loop
+    // spills (+2 us at configs[1])
+    int T_l = tc_layer_T<kLb>(a, g);
     // tell pass 2 (of this or a neighbouring CTA) that `n_done` more segments of group gi are in memory
     auto publish = [&]() {
       __threadfence();
@@ -301,7 +330,7 @@ __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const
       // half-full fourth row block: lanes 0-63 hold it on even tiles, lanes 64-127 on odd tiles (see the MMA warp)
       const bool shift = rs_valid > 384 && rs_valid <= 448 && rbl == 1;
       const bool act1_odd = lg >= 2 && 384 + (lg - 2) * 32 < rs_valid;
-      const int t_end = min(a.tpg, (x + 1) * kTcSegTiles);
+      const int t_end = min(tc_tiles_of<kLb>(a, T_l), (x + 1) * kTcSegTiles);
       for (int t = x * kTcSegTiles; t < t_end; ++t) {
         const int n_valid = T_l - (t * kTcTile + th * 64);
 #pragma unroll
@@ -356,7 +385,7 @@ __device__ __forceinline__ void tc_pass1(const TcSmem& s, const TcBars& b, const
         m0 = m1 = -INFINITY; z0 = z1 = 0.f;
       }
       ++n_done;
-      if (++x == a.spg) { publish(); x = 0; ++gi; g.next(a); if (kLb) T_l = layer_T(a.g, g.bl(a) % a.g.L, a.Tn); }
+      if (++x == tc_segs_of<kLb>(a, T_l)) { publish(); x = 0; ++gi; g.next(a); if (kLb) T_l = tc_layer_T<true>(a, g); }
     }
     if (n_done > 0) publish();
     st.as = as; st.aph = aph;
@@ -404,19 +433,21 @@ template <bool kEpi, bool kLb>
 __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const CUtensorMap* tmap_q, const CUtensorMap* tmap_k,
                                          const TcArgs& a, uint32_t tmem_base, TcRole& st) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int U = a.n_groups * a.tpg;
+  const int U = a.U2;
   const int u0 = tc_unit_begin(U, gridDim.x, blockIdx.x), u1 = tc_unit_begin(U, gridDim.x, blockIdx.x + 1);
 
   if (!kEpi && warp == 0) {
-    if (lane == 0) tc_producer<false>(s, b, tmap_q, tmap_k, a, u0, u1, st);
+    if (lane == 0) tc_producer<false, kLb>(s, b, tmap_q, tmap_k, a, u0, u1, st);
   } else if (!kEpi && warp == 1) {
     // ---------------- MMA issuer: the whole warp runs the loop, one elected lane issues ----------------
     const uint32_t q_lo = ptx::smem_desc_lo(ptx::smem_u32(s.q)), k_lo = ptx::smem_desc_lo(ptx::smem_u32(s.k));
     const uint32_t q_half16 = uint32_t(a.q_half_bytes) >> 4;
     int ks = st.ks, kph = st.kph, as = st.as, aph = st.aph, n_q = st.n_q;
     bool new_group = true;
-    int t = u0 % a.tpg;
-    TcCursor g; g.init(a, u0 / a.tpg);
+    int t, gi0;
+    tc_locate<kLb, false>(a, u0, gi0, t);
+    TcCursor g; g.init(a, gi0);
+    int T_l = tc_layer_T<kLb>(a, g);
     for (int u = u0; u < u1; ++u) {
       const int rs32 = (g.rs_valid(a) + 31) & ~31;
       if (new_group) { ptx::mbar_wait(b.q_full, n_q & 1); ++n_q; new_group = false; }
@@ -438,14 +469,14 @@ __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const
         __syncwarp();
         if (++as == 2) { as = 0; aph ^= 1; }
       }
-      const bool last_of_group = (u + 1 == u1) || t + 1 == a.tpg;
+      const bool last_of_group = (u + 1 == u1) || t + 1 == tc_tiles_of<kLb>(a, T_l);
       if (ptx::elect_one()) {
         ptx::mma_commit(&b.k_empty[ks]);
         if (last_of_group) ptx::mma_commit(b.q_empty);
       }
       __syncwarp();
       if (++ks == a.n_kst) { ks = 0; kph ^= 1; }
-      if (++t == a.tpg) { t = 0; g.next(a); new_group = true; }
+      if (++t == tc_tiles_of<kLb>(a, T_l)) { t = 0; g.next(a); new_group = true; if (kLb) T_l = tc_layer_T<true>(a, g); }
     }
   } else if (kEpi) {
     // ---------------- epilogue: one token per thread; warp (lane quarter lg, column quarter cq) ----------------
@@ -456,11 +487,12 @@ __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const
     float v[32];
     float acc[4] = {0.f, 0.f, 0.f, 0.f};
     bool new_group = true;
-    int t = u0 % a.tpg, rs32 = 0, gi = u0 / a.tpg, T_l = a.Tn;
+    int t, gi, rs32 = 0, T_l = a.Tn;
+    tc_locate<kLb, false>(a, u0, gi, t);
     float* col = nullptr;                                                // this warp's column-sum slot of the group
     TcCursor g; g.init(a, gi);
     // seg_cnt[group] counts 16 (epilogue warps) per finished pass-1 segment of THIS update: k_append zeroes the counters
-    const unsigned seg_target = unsigned(a.spg) * kTcEpiWarps;
+    // (layer-dependent budgets: of the group's layer, spg_l segments)
     // sum over the 32 probe rows [col0, col0 + 32) of this token (32 registers live: no spills in this loop --
     // a local-memory load would queue behind the exp2 traffic like every other MIO instruction)
     auto fold = [&](int col0) {
@@ -482,7 +514,9 @@ __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const
       if (new_group) {
         // all pass-1 segments of the group must be in memory (they come from this CTA and its schedule
         // neighbours, none of which ever waits during pass 1, and every CTA of the grid is resident)
+        if (kLb) T_l = tc_layer_T<true>(a, g);
         if (lane == 0) {
+          const unsigned seg_target = unsigned(tc_segs_of<kLb>(a, T_l)) * kTcEpiWarps;
           unsigned seen;
           do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(a.g.seg_cnt + gi) : "memory"); }
           while (seen < seg_target);
@@ -491,11 +525,10 @@ __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const
         ptx::named_bar_sync(1, kTcEpiWarps * 32);                        // everyone is done with the old c_r
         const int bl = g.bl(a), rows_total = a.g.Hq * a.g.p_max;
         tc_merge_rows(reinterpret_cast<const float2*>(a.g.partial) + size_t(bl) * a.spg * rows_total + g.stat_row0(a),
-                      a.spg, rows_total, g.rs_valid(a), s.c, threadIdx.x - kTcCtlWarps * 32, g.sc * a.RS, a.P,
+                      tc_segs_of<kLb>(a, T_l), rows_total, g.rs_valid(a), s.c, threadIdx.x - kTcCtlWarps * 32, g.sc * a.RS, a.P,
                       g.ls >= a.g.L - a.g.n_shallow - a.g.n_deep ? a.g.probe_deep_begin : 0);
         ptx::named_bar_sync(1, kTcEpiWarps * 32);
         rs32 = (g.rs_valid(a) + 31) & ~31;
-        if (kLb) T_l = layer_T(a.g, bl % a.g.L, a.Tn);
         col = a.g.colsum + (size_t(bl) * a.g.n_vh_max + (g.kvh * a.n_sc + g.sc) * 4 + cq) * a.g.cap;
         new_group = false;
       }
@@ -523,7 +556,7 @@ __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const
       const int tok = t * kTcTile + tok_in_tile;
       if (tok < T_l) col[tok] = (acc[0] + acc[1]) + (acc[2] + acc[3]);
       acc[0] = acc[1] = acc[2] = acc[3] = 0.f;
-      if (++t == a.tpg) { t = 0; ++gi; g.next(a); new_group = true; }
+      if (++t == tc_tiles_of<kLb>(a, T_l)) { t = 0; ++gi; g.next(a); new_group = true; }
     }
   }
 }
@@ -719,8 +752,28 @@ inline int tc_score(hermes_t* h, const void* q_probe, int Tn, int n_new, int P, 
   a.n_groups = g.B * (g.L - g.n_shallow) * g.Hkv * a.n_sc;
   a.tpg = (Tn + kTcTile - 1) / kTcTile;
   a.spg = (a.tpg + kTcSegTiles - 1) / kTcSegTiles;
-  const long long U1 = (long long)a.n_groups * a.spg, U2 = (long long)a.n_groups * a.tpg;
+  long long U1 = (long long)a.n_groups * a.spg, U2 = (long long)a.n_groups * a.tpg;
   if (U2 > INT_MAX / 2) { h->err = "tcgen05 scoring: too many (group, tile) units"; return HERMES_ECAPACITY; }
+  if (h->lb) {
+    // layer-dependent budgets: Tn is the largest scored layer's count (it sizes the partial-slot stride a.spg); every scored
+    // layer runs its own ceil(T_l / 128) tiles, and the CTAs split the sums of those.  Prefix sums per (stream, scored layer)
+    // block of Hkv * n_sc groups, uploaded stream-ordered (pageable source: staged when the call returns)
+    const int Ls = g.L - g.n_shallow, nb = g.B * Ls, ngb = g.Hkv * a.n_sc;
+    std::vector<int32_t> pre(2 * size_t(nb + 1), 0);
+    for (int i = 0; i < nb; ++i) {
+      const int T_l = h->lay_len[g.n_shallow + i % Ls] + n_new;
+      const int tiles = (T_l + kTcTile - 1) / kTcTile, segs = (tiles + kTcSegTiles - 1) / kTcSegTiles;
+      pre[i + 1] = pre[i] + ngb * segs;
+      pre[nb + 1 + i + 1] = pre[nb + 1 + i] + ngb * tiles;
+    }
+    U1 = pre[nb]; U2 = pre[2 * nb + 1];
+    int32_t* dev = reinterpret_cast<int32_t*>(h->ws + h->lay.tc_pre);
+    if (cudaMemcpyAsync(dev, pre.data(), pre.size() * 4, cudaMemcpyHostToDevice, s) != cudaSuccess) {
+      h->err = "tcgen05 scoring: upload of the per-layer schedule failed"; return HERMES_ECUDA;
+    }
+    a.pre_s = dev; a.pre_t = dev + nb + 1;
+  }
+  a.U1 = int(U1); a.U2 = int(U2);
   // every CTA must be resident (pass 2 waits on pass-1 progress of other CTAs): at most one CTA per SM
   const int n_cta = int(std::min<long long>(st->n_sm, U1));
   if (a.spg > h->lay.n_part_max || g.Hkv * a.n_sc * 4 > g.n_vh_max || a.n_groups > g.B * g.L * g.n_vh_max) { h->err = "internal: tc scratch too small"; return HERMES_ESTATE; }
