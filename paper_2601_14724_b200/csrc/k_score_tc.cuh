@@ -491,8 +491,8 @@ __device__ __forceinline__ void tc_pass2(const TcSmem& s, const TcBars& b, const
     tc_locate<kLb, false>(a, u0, gi, t);
     float* col = nullptr;                                                // this warp's column-sum slot of the group
     TcCursor g; g.init(a, gi);
-    // seg_cnt[group] counts 16 (epilogue warps) per finished pass-1 segment of THIS update: k_append zeroes the counters
-    // (layer-dependent budgets: of the group's layer, spg_l segments)
+    // seg_cnt[group] counts 16 (epilogue warps) per finished pass-1 segment of THIS update (k_append zeroes the counters);
+    // a group is complete at 16 x its segment count (layer-dependent budgets: its layer's own)
     // sum over the 32 probe rows [col0, col0 + 32) of this token (32 registers live: no spills in this loop --
     // a local-memory load would queue behind the exp2 traffic like every other MIO instruction)
     auto fold = [&](int col0) {
