@@ -199,3 +199,61 @@ def test_summary_token_with_layer_budgets_on_tcgen05():
     m, lens, n_cmp, _, paths = _run(wl, (1.3, 1.0, 0.7), 9, oover=dict(summary_token=True), summary_token=1,
                                     score_path=hb.HERMES_SCORE_TCGEN05)
     assert lens == np.minimum(m, 196 * 9).tolist() and paths == {hb.HERMES_SCORE_TCGEN05} and _run.n_summ >= 8
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_random_geometry_with_layer_budgets(seed):
+    """Seeded random geometries and weightings (ragged sizes, 1-4 KV heads, probe counts across the 512-row super-chunk
+    boundary) through the same lock-step comparison; even seeds force the tcgen05 path and its per-layer tile schedule."""
+    r = np.random.default_rng(500 + seed)
+    tc = seed % 2 == 0
+    hkv, grp = int(r.choice([1, 2, 3, 4])), int(r.choice([2, 4, 7]))
+    wl = CONFIGS["llava_ov_7b"].scaled(n_layers=int(r.integers(4, 9)), n_kv_heads=hkv, n_q_heads=hkv * grp,
+                                       budget=int(r.integers(600, 1100)), chunk_tokens=int(r.integers(40, 230)),
+                                       probe_tokens=int(r.integers(max(1, -(-32 // grp)), 100)), seed=8100 + seed)
+    w = tuple(float(x) for x in np.round(r.uniform(0.6, 1.7, 3), 2))
+    summ = bool(r.integers(0, 2))
+    over = dict(score_path=hb.HERMES_SCORE_TCGEN05 if tc else hb.HERMES_SCORE_SIMT)
+    oover = {}
+    if summ:
+        over.update(summary_token=1); oover.update(summary_token=True)
+    n_up = int(np.ceil(max(ho.layer_budgets(oracle_config(wl, budget_weights=w, capacity=0)).max() / wl.chunk_tokens, 1))) + 4
+    m, lens, n_cmp, _, paths = _run(wl, w, n_up, oover=oover, **over)
+    assert lens == m.tolist() and n_cmp >= wl.n_layers, (wl, w, summ)
+    assert paths == {hb.HERMES_SCORE_TCGEN05 if tc else hb.HERMES_SCORE_SIMT}
+
+
+def test_two_streams_with_layer_budgets_equal_two_single_stream_handles():
+    """The per-layer schedule tables of k_tc_score<true> are per (stream, scored layer): a 2-stream handle must leave, for
+    each stream, exactly the cache a single-stream handle leaves for the same inputs (bit for bit), V move riding or not."""
+    wl = CONFIGS["llava_ov_7b"].scaled(n_layers=7, budget=896, probe_tokens=40)
+    w = (0.7, 1.6, 0.7)
+    gen = torch.Generator(device="cuda").manual_seed(77)
+    L, Hkv, Hq, d, C, P = wl.n_layers, wl.n_kv_heads, wl.n_q_heads, wl.head_dim, wl.chunk_tokens, wl.probe_tokens
+    steps = [(torch.randn(2, L, C, Hkv, d, generator=gen, device="cuda").to(torch.bfloat16),
+              torch.randn(2, L, C, Hkv, d, generator=gen, device="cuda").to(torch.bfloat16),
+              torch.randn(2, L, Hq, P, d, generator=gen, device="cuda").to(torch.bfloat16)) for _ in range(12)]
+
+    def run(n_streams, pick):
+        cfg = hb.config_for_workload(wl.scaled(n_streams=n_streams), budget_weight=w, max_tokens=0,
+                                     score_path=hb.HERMES_SCORE_TCGEN05)
+        h = hb.hermes_create(cfg)
+        for i, (K, V, Q) in enumerate(steps):
+            K, V, Q = (x[pick].contiguous() for x in (K, V, Q))
+            hb.hermes_append_chunk(h, K, V, Q if i >= 3 else None)
+        torch.cuda.synchronize()
+        out = []
+        for b in range(n_streams):
+            for l in range(L):
+                v = hb.hermes_get_cache(h, b, l)
+                out.append({k: v[k].clone() for k in ("k", "v", "pos", "last_kept", "last_scores")})
+        torch.cuda.synchronize()
+        assert hb.hermes_device_status(h) == 0 and hb.hermes_last_score_path(h) == hb.HERMES_SCORE_TCGEN05
+        hb.hermes_destroy(h)
+        return out
+
+    both = run(2, slice(0, 2))
+    singles = run(1, slice(0, 1)) + run(1, slice(1, 2))
+    for i, (a, b) in enumerate(zip(both, singles)):
+        for k in a:
+            assert torch.equal(a[k], b[k]), f"stream {i // L} layer {i % L}: {k} differs"
