@@ -277,7 +277,12 @@ def run_ours(args, backend=None, hb=None):
     for i in range(3):
         host_step(i)
     ms_e2e = timed(n_e2e, host_step)
-    h2d = sum(x.numel() * x.element_size() for x in host_pool[0])
+    # bytes the library moves per call: K, V and the probe slices of the scored layers (shallow layers' slices are never read;
+    # n_shallow defaults to max(1, round(0.1 L)), include/hermes.h)
+    n_shallow = max(1, (wl.n_layers + 5) // 10)
+    Kh, Vh, Qh = host_pool[0]
+    h2d = (Kh.numel() * Kh.element_size() + Vh.numel() * Vh.element_size()
+           + Qh.numel() * Qh.element_size() * (wl.n_layers - n_shallow) // wl.n_layers)
     d2h = 0 if lb else kept_host[0].numel() * 4
     rides = bool(hb.hermes_v_pending(h))
 

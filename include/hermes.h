@@ -156,9 +156,9 @@ int hermes_create(const hermes_config *cfg, void *workspace, size_t bytes, herme
 int hermes_append_chunk(hermes_t *h, const void *K_new, const void *V_new, const void *Q_probe,
                         int32_t n_new, int32_t n_probe, int32_t pos_start, void *cuda_stream);
 
-/* Same update with HOST buffers (pinned memory recommended), which must hold their data when the call is made: Q_probe,
- * K_new and then V_new are copied to the device with cudaMemcpyAsync on a library-owned copy stream (created on first
- * use) into one of two staging sets, so the copies of a call overlap the kernels of the call before it; `cuda_stream`
+/* Same update with HOST buffers (pinned memory recommended), which must hold their data when the call is made: Q_probe
+ * (the slices of the scored layers only), K_new and then V_new are copied to the device with cudaMemcpyAsync on a
+ * library-owned copy stream (created on first use) into one of two staging sets, so the copies of a call overlap the kernels of the call before it; `cuda_stream`
  * waits for K before the update's kernels and for V before the V rows are appended, so everything the call enqueues is
  * ordered on `cuda_stream` when it returns.  If kept_out != NULL, copies the kept index lists I_l [B, L, budget] int32
  * back to the host on `cuda_stream` (only meaningful when an eviction ran; not available with layer-dependent budgets).

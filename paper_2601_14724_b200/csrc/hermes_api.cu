@@ -585,7 +585,13 @@ extern "C" int hermes_append_chunk_host(hermes_t* h, const void* K_host, const v
   }
   cudaStream_t cs = h->side_stream;
   if (h->ev_free_set[p]) CUDA_TRY(h, cudaStreamWaitEvent(cs, h->ev_free[p], 0));   // the call before the last is done with set p
-  if (Q_host) CUDA_TRY(h, cudaMemcpyAsync(sq, Q_host, BL * c.n_q_heads * n_probe * c.head_dim * h->lay.esize, cudaMemcpyHostToDevice, cs));
+  if (Q_host) {
+    // the probe slices of shallow layers are never read (include/hermes.h): per stream, copy layers [n_shallow, L) only
+    const size_t lq = size_t(c.n_q_heads) * n_probe * c.head_dim * h->lay.esize, ns = size_t(h->lay.n_shallow);
+    if (c.n_layers > int(ns))
+      CUDA_TRY(h, cudaMemcpy2DAsync(sq + ns * lq, c.n_layers * lq, static_cast<const char*>(Q_host) + ns * lq, c.n_layers * lq,
+                                    (c.n_layers - ns) * lq, size_t(c.n_streams), cudaMemcpyHostToDevice, cs));
+  }
   CUDA_TRY(h, cudaMemcpyAsync(sk, K_host, kv_bytes, cudaMemcpyHostToDevice, cs));
   CUDA_TRY(h, cudaEventRecord(h->ev_k_done[p], cs));
   CUDA_TRY(h, cudaMemcpyAsync(sv, V_host, kv_bytes, cudaMemcpyHostToDevice, cs));
